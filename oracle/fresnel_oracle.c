@@ -1,0 +1,362 @@
+/*
+ * fresnel_oracle.c -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+ *
+ * A plain, slow, obviously-correct CPU restatement of the plane-to-plane Fresnel
+ * propagation hot path that arXiv 1806.06467 (Douglas & Perrin) accelerates in POPPY.
+ * It exists so that the CUDA library in paper_1806_06467_b200/csrc can be checked
+ * against something independent.  Only tests/, __graft_entry__.smoke() and the
+ * cpu_baseline / --impl reference legs of bench.py may load this file's library.  It
+ * shares no code, header, table or constant generator with the CUDA path.
+ *
+ * Arithmetic: double for the field, long double (x87 80-bit) for every phase.
+ * No blocking, fusion or reordering beyond what the definitions below state:
+ * the fftshift/ifftshift calls are literal array rotations, the chirps are evaluated
+ * per pixel from r^2 = x^2 + y^2 (the non-separable route), the 2-D transform is a
+ * textbook iterative radix-2 FFT applied to rows and then to columns.
+ *
+ * Passages followed (PAPER.md line numbers; DESIGN.md lists every reading g1..g20):
+ *   - the three bottlenecks FFT / complex exponentials / fftshift:   PAPER.md:77-81 (sec. 2.1)
+ *   - quadratic phase factor exp[i(x^2+y^2)/z], Eq. 2:
+ *       read as exp(i*pi*(x^2+y^2)/(lambda*z))  (reading g1; thin lens f => z = -f, g2)
+ *   - optic phasor A*exp[2*pi*i/lambda * phi], Eq. 3:
+ *   - "plane-to-plane angular spectrum propagation ... thin lenses":
+ *       transfer function exp(-i*pi*lambda*z*(fx^2+fy^2)) from BASELINE.json:north_star (g4)
+ *   - "direct Fresnel" single-FFT propagation, pixelscale changes:
+ *   - fftshift puts the origin in the centre of the array:
+ *
+ * Parity pins: every function here is pinned in tests/test_oracle_pins.py (P0..P13 of
+ * DESIGN.md) against closed forms / exact identities / brute force.  Nothing is
+ * "parity unpinned".
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#define ORACLE_OK 0
+#define ORACLE_ERR_INVALID_ARG 1
+#define ORACLE_ERR_UNSUPPORTED 2
+#define ORACLE_ERR_ALLOC 3
+
+static const long double PI_L = 3.14159265358979323846264338327950288419716939937510L;
+
+static int g_threads = 0; /* 0 = OpenMP default */
+
+void oracle_set_threads(int n) { g_threads = n > 0 ? n : 0; }
+
+int oracle_get_threads(void)
+{
+#ifdef _OPENMP
+    return g_threads > 0 ? g_threads : omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+static int nthreads(void) { return oracle_get_threads(); }
+
+static int is_pow2(int n) { return n > 0 && (n & (n - 1)) == 0; }
+
+/* ------------------------------------------------------------------------------------------
+ * 1. dft2_naive: the literal O(N^4) double sum  (DESIGN.md oracle item 1)
+ *      out[p,q] = sum_j sum_k u[j,k] * exp(sign * 2*pi*i * (j*p + k*q) / N)
+ *    sign = -1: unnormalised forward transform;  sign = +1: inverse, scaled by 1/N^2 (g6).
+ *    The root exp(sign*2*pi*i*m/N) is taken from direct cosl/sinl of the reduced integer m.
+ * ------------------------------------------------------------------------------------------ */
+int oracle_dft2_naive(double *u, int N, int sign)
+{
+    if (!u || N <= 0 || (sign != 1 && sign != -1)) return ORACLE_ERR_INVALID_ARG;
+    if (N > 64) return ORACLE_ERR_UNSUPPORTED;
+    size_t n2 = (size_t)N * N;
+    double *in = (double *)malloc(2 * n2 * sizeof(double));
+    double *wr = (double *)malloc(N * sizeof(double));
+    double *wi = (double *)malloc(N * sizeof(double));
+    if (!in || !wr || !wi) { free(in); free(wr); free(wi); return ORACLE_ERR_ALLOC; }
+    memcpy(in, u, 2 * n2 * sizeof(double));
+    for (int m = 0; m < N; ++m) {
+        long double a = (long double)sign * 2.0L * PI_L * (long double)m / (long double)N;
+        wr[m] = (double)cosl(a);
+        wi[m] = (double)sinl(a);
+    }
+#pragma omp parallel for num_threads(nthreads()) schedule(static)
+    for (int p = 0; p < N; ++p) {
+        for (int q = 0; q < N; ++q) {
+            double sr = 0.0, si = 0.0;
+            for (int j = 0; j < N; ++j) {
+                for (int k = 0; k < N; ++k) {
+                    int m = (int)(((long)j * p + (long)k * q) % N);
+                    double ar = in[2 * ((size_t)j * N + k)], ai = in[2 * ((size_t)j * N + k) + 1];
+                    sr += ar * wr[m] - ai * wi[m];
+                    si += ar * wi[m] + ai * wr[m];
+                }
+            }
+            if (sign > 0) { sr /= (double)N * (double)N; si /= (double)N * (double)N; }
+            u[2 * ((size_t)p * N + q)] = sr;
+            u[2 * ((size_t)p * N + q) + 1] = si;
+        }
+    }
+    free(in); free(wr); free(wi);
+    return ORACLE_OK;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * 2. fft2: own iterative radix-2 (bit reversal + log2 N butterfly stages), rows then columns.
+ *    Twiddles come from direct cosl/sinl per index, never from a recurrence.
+ * ------------------------------------------------------------------------------------------ */
+static void make_twiddles(double *tw, int n, int sign)
+{
+    for (int k = 0; k < n / 2; ++k) {
+        long double a = (long double)sign * 2.0L * PI_L * (long double)k / (long double)n;
+        tw[2 * k] = (double)cosl(a);
+        tw[2 * k + 1] = (double)sinl(a);
+    }
+}
+
+static void fft1d_radix2(double *x, int n, const double *tw)
+{
+    /* bit-reversal permutation */
+    for (int i = 1, j = 0; i < n; ++i) {
+        int bit = n >> 1;
+        for (; j & bit; bit >>= 1) j ^= bit;
+        j ^= bit;
+        if (i < j) {
+            double tr = x[2 * i], ti = x[2 * i + 1];
+            x[2 * i] = x[2 * j]; x[2 * i + 1] = x[2 * j + 1];
+            x[2 * j] = tr; x[2 * j + 1] = ti;
+        }
+    }
+    for (int len = 2; len <= n; len <<= 1) {
+        int half = len >> 1, step = n / len;
+        for (int i = 0; i < n; i += len) {
+            for (int k = 0; k < half; ++k) {
+                double wr = tw[2 * (k * step)], wi = tw[2 * (k * step) + 1];
+                double *a = x + 2 * (i + k), *b = x + 2 * (i + k + half);
+                double br = b[0] * wr - b[1] * wi;
+                double bi = b[0] * wi + b[1] * wr;
+                b[0] = a[0] - br; b[1] = a[1] - bi;
+                a[0] = a[0] + br; a[1] = a[1] + bi;
+            }
+        }
+    }
+}
+
+/* normalise != 0: multiply by 1/N^2 (only meaningful with sign = +1). */
+static int fft2_core(double *u, int N, int sign, int normalise)
+{
+    if (!u || (sign != 1 && sign != -1)) return ORACLE_ERR_INVALID_ARG;
+    if (!is_pow2(N) || N < 2) return ORACLE_ERR_UNSUPPORTED;
+    double *tw = (double *)malloc((size_t)N * sizeof(double));
+    if (!tw) return ORACLE_ERR_ALLOC;
+    make_twiddles(tw, N, sign);
+    int fail = 0;
+#pragma omp parallel num_threads(nthreads())
+    {
+        double *col = (double *)malloc(2 * (size_t)N * sizeof(double));
+        if (!col) {
+#pragma omp atomic write
+            fail = 1;
+        }
+#pragma omp barrier
+        if (!fail) {
+#pragma omp for schedule(static)
+            for (int j = 0; j < N; ++j) fft1d_radix2(u + 2 * (size_t)j * N, N, tw);
+#pragma omp for schedule(static)
+            for (int k = 0; k < N; ++k) {
+                for (int j = 0; j < N; ++j) {
+                    col[2 * j] = u[2 * ((size_t)j * N + k)];
+                    col[2 * j + 1] = u[2 * ((size_t)j * N + k) + 1];
+                }
+                fft1d_radix2(col, N, tw);
+                for (int j = 0; j < N; ++j) {
+                    u[2 * ((size_t)j * N + k)] = col[2 * j];
+                    u[2 * ((size_t)j * N + k) + 1] = col[2 * j + 1];
+                }
+            }
+            if (normalise) {
+                double s = 1.0 / ((double)N * (double)N);
+#pragma omp for schedule(static)
+                for (int j = 0; j < N; ++j)
+                    for (int k = 0; k < 2 * N; ++k) u[2 * (size_t)j * N + k] *= s;
+            }
+        }
+        free(col);
+    }
+    free(tw);
+    return fail ? ORACLE_ERR_ALLOC : ORACLE_OK;
+}
+
+/* forward (sign=-1) unnormalised; inverse (sign=+1) scaled by 1/N^2 (reading g6). */
+int oracle_fft2(double *u, int N, int sign) { return fft2_core(u, N, sign, sign > 0); }
+
+/* ------------------------------------------------------------------------------------------
+ * literal shifts: fftshift(x)[i] = x[(i - N/2) mod N], ifftshift(x)[i] = x[(i + N/2) mod N]
+ * ------------------------------------------------------------------------------------------ */
+static int roll2d(double *u, int N, int s)
+{
+    size_t n2 = (size_t)N * N;
+    double *t = (double *)malloc(2 * n2 * sizeof(double));
+    if (!t) return ORACLE_ERR_ALLOC;
+    memcpy(t, u, 2 * n2 * sizeof(double));
+    s = ((s % N) + N) % N;
+#pragma omp parallel for num_threads(nthreads()) schedule(static)
+    for (int j = 0; j < N; ++j) {
+        int jj = (j + s) % N;
+        for (int k = 0; k < N; ++k) {
+            int kk = (k + s) % N;
+            u[2 * ((size_t)jj * N + kk)] = t[2 * ((size_t)j * N + k)];
+            u[2 * ((size_t)jj * N + kk) + 1] = t[2 * ((size_t)j * N + k) + 1];
+        }
+    }
+    free(t);
+    return ORACLE_OK;
+}
+
+int oracle_fftshift(double *u, int N) { return (!u || N <= 0) ? ORACLE_ERR_INVALID_ARG : roll2d(u, N, N / 2); }
+int oracle_ifftshift(double *u, int N) { return (!u || N <= 0) ? ORACLE_ERR_INVALID_ARG : roll2d(u, N, -(N / 2)); }
+
+/* fft2d as the ABI exposes it: forward unnormalised, inverse x 1/N^2;
+ * centered != 0  =>  fftshift o fft2 o ifftshift  (origin on pixel N/2, reading g8). */
+int oracle_fft2d(double *u, int N, int direction, int centered)
+{
+    int sign = direction > 0 ? -1 : +1; /* FRESNEL_FORWARD=+1 uses kernel exp(-...), INVERSE=-1 uses exp(+...) */
+    if (direction != 1 && direction != -1) return ORACLE_ERR_INVALID_ARG;
+    int rc;
+    if (centered && (rc = oracle_ifftshift(u, N)) != ORACLE_OK) return rc;
+    if ((rc = oracle_fft2(u, N, sign)) != ORACLE_OK) return rc;
+    if (centered && (rc = oracle_fftshift(u, N)) != ORACLE_OK) return rc;
+    return ORACLE_OK;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * 3. apply_qpf (Eq. 2, reading g1):
+ *      u[j,k] *= exp(i*pi*(x_k^2 + y_j^2)/(lambda*z)),  x_k = (k-N/2)*dx, y_j = (j-N/2)*dx
+ *    per pixel, r^2 and the phase in long double.  A thin lens of focal length f is z = -f (g2).
+ * ------------------------------------------------------------------------------------------ */
+int oracle_apply_qpf(double *u, int N, double dx, double lambda, double z)
+{
+    if (!u || N <= 0 || !(dx > 0) || !(lambda > 0) || !isfinite(z) || z == 0.0) return ORACLE_ERR_INVALID_ARG;
+    long double ldx = dx, ll = lambda, lz = z;
+#pragma omp parallel for num_threads(nthreads()) schedule(static)
+    for (int j = 0; j < N; ++j) {
+        long double y = (long double)(j - N / 2) * ldx;
+        for (int k = 0; k < N; ++k) {
+            long double x = (long double)(k - N / 2) * ldx;
+            long double r2 = x * x + y * y;
+            long double th = PI_L * r2 / (ll * lz);
+            double c = (double)cosl(th), s = (double)sinl(th);
+            double *p = u + 2 * ((size_t)j * N + k);
+            double re = p[0] * c - p[1] * s, im = p[0] * s + p[1] * c;
+            p[0] = re; p[1] = im;
+        }
+    }
+    return ORACLE_OK;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * 4. apply_mask (Eq. 3, reading g3):  u *= A * exp(i*2*pi*OPD/lambda)
+ *    amp and/or opd may be NULL (A = 1, OPD = 0).
+ * ------------------------------------------------------------------------------------------ */
+int oracle_apply_mask(double *u, int N, const double *amp, const double *opd, double lambda)
+{
+    if (!u || N <= 0 || !(lambda > 0)) return ORACLE_ERR_INVALID_ARG;
+    long double ll = lambda;
+#pragma omp parallel for num_threads(nthreads()) schedule(static)
+    for (int j = 0; j < N; ++j) {
+        for (int k = 0; k < N; ++k) {
+            size_t i = (size_t)j * N + k;
+            double a = amp ? amp[i] : 1.0;
+            double c = 1.0, s = 0.0;
+            if (opd) {
+                long double th = 2.0L * PI_L * (long double)opd[i] / ll;
+                c = (double)cosl(th); s = (double)sinl(th);
+            }
+            double re = u[2 * i] * c - u[2 * i + 1] * s, im = u[2 * i] * s + u[2 * i + 1] * c;
+            u[2 * i] = a * re; u[2 * i + 1] = a * im;
+        }
+    }
+    return ORACLE_OK;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * 5. propagate_as: the literal sequence  ifftshift -> fft2(-) -> x H -> fft2(+) -> fftshift
+ *      H[p,q] = exp(-i*pi*lambda*z*(f_q^2 + f_p^2)),  f in FFT order: f_q = q/(N dx) (q < N/2),
+ *      (q-N)/(N dx) otherwise.  No piston exp(ikz) (g5).  z = 0 is the identity (g11).
+ *    ("plane-to-plane angular spectrum propagation"; BASELINE.json:north_star)
+ * ------------------------------------------------------------------------------------------ */
+int oracle_propagate_as(double *u, int N, double dx, double lambda, double z)
+{
+    if (!u || N <= 0 || !(dx > 0) || !(lambda > 0) || !isfinite(z)) return ORACLE_ERR_INVALID_ARG;
+    if (!is_pow2(N)) return ORACLE_ERR_UNSUPPORTED;
+    int rc;
+    if ((rc = oracle_ifftshift(u, N)) != ORACLE_OK) return rc;
+    if ((rc = oracle_fft2(u, N, -1)) != ORACLE_OK) return rc;
+    long double ldx = dx, ll = lambda, lz = z;
+#pragma omp parallel for num_threads(nthreads()) schedule(static)
+    for (int p = 0; p < N; ++p) {
+        long double fp = (long double)(p < N / 2 ? p : p - N) / ((long double)N * ldx);
+        for (int q = 0; q < N; ++q) {
+            long double fq = (long double)(q < N / 2 ? q : q - N) / ((long double)N * ldx);
+            long double th = -PI_L * ll * lz * (fq * fq + fp * fp);
+            double c = (double)cosl(th), s = (double)sinl(th);
+            double *e = u + 2 * ((size_t)p * N + q);
+            double re = e[0] * c - e[1] * s, im = e[0] * s + e[1] * c;
+            e[0] = re; e[1] = im;
+        }
+    }
+    if ((rc = oracle_fft2(u, N, +1)) != ORACLE_OK) return rc;
+    if ((rc = oracle_fftshift(u, N)) != ORACLE_OK) return rc;
+    return ORACLE_OK;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * 6. propagate_direct (single-FFT Fresnel; readings g7, g10):
+ *      u *= Q_dx(z);  centred transform by literal ifftshift / fft2 / fftshift
+ *      (forward kernel if z > 0, unnormalised inverse kernel, i.e. N^2 * ifft2, if z < 0);
+ *      u *= dx^2/(i*lambda*z);   dx' = lambda*|z|/(N*dx);   u *= Q_dx'(z).
+ * ------------------------------------------------------------------------------------------ */
+int oracle_propagate_direct(double *u, int N, double *dx_inout, double lambda, double z)
+{
+    if (!u || !dx_inout || N <= 0 || !(*dx_inout > 0) || !(lambda > 0) || !isfinite(z) || z == 0.0)
+        return ORACLE_ERR_INVALID_ARG;
+    if (!is_pow2(N)) return ORACLE_ERR_UNSUPPORTED;
+    double dx = *dx_inout;
+    int rc;
+    if ((rc = oracle_apply_qpf(u, N, dx, lambda, z)) != ORACLE_OK) return rc;
+    if ((rc = oracle_ifftshift(u, N)) != ORACLE_OK) return rc;
+    if ((rc = fft2_core(u, N, z > 0 ? -1 : +1, 0)) != ORACLE_OK) return rc;
+    if ((rc = oracle_fftshift(u, N)) != ORACLE_OK) return rc;
+    /* dx^2/(i lambda z) = -i * dx^2/(lambda z) */
+    long double g = (long double)dx * (long double)dx / ((long double)lambda * (long double)z);
+    double gd = (double)g;
+#pragma omp parallel for num_threads(nthreads()) schedule(static)
+    for (int j = 0; j < N; ++j) {
+        for (int k = 0; k < N; ++k) {
+            double *e = u + 2 * ((size_t)j * N + k);
+            double re = e[1] * gd, im = -e[0] * gd; /* (re + i im) * (-i g) = im*g - i re*g */
+            e[0] = re; e[1] = im;
+        }
+    }
+    long double dxo = (long double)lambda * fabsl((long double)z) / ((long double)N * (long double)dx);
+    double dx_out = (double)dxo;
+    if ((rc = oracle_apply_qpf(u, N, dx_out, lambda, z)) != ORACLE_OK) return rc;
+    *dx_inout = dx_out;
+    return ORACLE_OK;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * fused surface = thin lens f  (QPF with z = -f; f = +-INFINITY => no lens), then the optic
+ * phasor, then angular-spectrum propagation by z; applied literally one after the other
+ * ("add_optic(lens, distance=...)").
+ * ------------------------------------------------------------------------------------------ */
+int oracle_surface_as(double *u, int N, double dx, double lambda, double f,
+                      const double *amp, const double *opd, double z)
+{
+    int rc;
+    if (isnan(f) || f == 0.0) return ORACLE_ERR_INVALID_ARG;
+    if (isfinite(f) && (rc = oracle_apply_qpf(u, N, dx, lambda, -f)) != ORACLE_OK) return rc;
+    if ((amp || opd) && (rc = oracle_apply_mask(u, N, amp, opd, lambda)) != ORACLE_OK) return rc;
+    return oracle_propagate_as(u, N, dx, lambda, z);
+}

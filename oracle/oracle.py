@@ -1,0 +1,168 @@
+"""ctypes face of oracle/liboracle.so (TEST INFRASTRUCTURE -- see fresnel_oracle.c header).
+
+Every function takes/returns numpy complex128 arrays of shape (N, N) (or (batch, N, N) for the
+``*_batch`` helpers, which just loop) and never touches the GPU.  Citations are in the C file.
+"""
+import ctypes
+import math
+
+import numpy as np
+
+from . import build as _build
+
+_lib = None
+
+ORACLE_OK = 0
+FORWARD = +1
+INVERSE = -1
+
+
+class OracleError(RuntimeError):
+    pass
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        path = _build.build()
+        L = ctypes.CDLL(path)
+        dp = ctypes.POINTER(ctypes.c_double)
+        L.oracle_set_threads.argtypes = [ctypes.c_int]
+        L.oracle_set_threads.restype = None
+        L.oracle_get_threads.argtypes = []
+        L.oracle_get_threads.restype = ctypes.c_int
+        L.oracle_dft2_naive.argtypes = [dp, ctypes.c_int, ctypes.c_int]
+        L.oracle_fft2.argtypes = [dp, ctypes.c_int, ctypes.c_int]
+        L.oracle_fftshift.argtypes = [dp, ctypes.c_int]
+        L.oracle_ifftshift.argtypes = [dp, ctypes.c_int]
+        L.oracle_fft2d.argtypes = [dp, ctypes.c_int, ctypes.c_int, ctypes.c_int]
+        L.oracle_apply_qpf.argtypes = [dp, ctypes.c_int, ctypes.c_double, ctypes.c_double, ctypes.c_double]
+        L.oracle_apply_mask.argtypes = [dp, ctypes.c_int, dp, dp, ctypes.c_double]
+        L.oracle_propagate_as.argtypes = [dp, ctypes.c_int, ctypes.c_double, ctypes.c_double, ctypes.c_double]
+        L.oracle_propagate_direct.argtypes = [dp, ctypes.c_int, dp, ctypes.c_double, ctypes.c_double]
+        L.oracle_surface_as.argtypes = [dp, ctypes.c_int, ctypes.c_double, ctypes.c_double, ctypes.c_double,
+                                        dp, dp, ctypes.c_double]
+        for name in ("oracle_dft2_naive", "oracle_fft2", "oracle_fftshift", "oracle_ifftshift", "oracle_fft2d",
+                     "oracle_apply_qpf", "oracle_apply_mask", "oracle_propagate_as", "oracle_propagate_direct",
+                     "oracle_surface_as"):
+            getattr(L, name).restype = ctypes.c_int
+        _lib = L
+    return _lib
+
+
+def set_threads(n: int) -> None:
+    lib().oracle_set_threads(int(n))
+
+
+def get_threads() -> int:
+    return int(lib().oracle_get_threads())
+
+
+def _prep(u):
+    a = np.array(u, dtype=np.complex128, order="C", copy=True)
+    if a.ndim != 2 or a.shape[0] != a.shape[1]:
+        raise ValueError("oracle expects a square (N, N) array")
+    return a, a.shape[0]
+
+
+def _dptr(a):
+    return a.ctypes.data_as(ctypes.POINTER(ctypes.c_double))
+
+
+def _real(m, N):
+    if m is None:
+        return None, None
+    a = np.ascontiguousarray(m, dtype=np.float64)
+    if a.shape != (N, N):
+        raise ValueError("map must be (N, N)")
+    return a, _dptr(a)
+
+
+def _check(rc, what):
+    if rc != ORACLE_OK:
+        raise OracleError(f"{what} failed with oracle status {rc}")
+
+
+def dft2_naive(u, sign):
+    a, N = _prep(u)
+    _check(lib().oracle_dft2_naive(_dptr(a), N, int(sign)), "dft2_naive")
+    return a
+
+
+def fft2(u, sign):
+    a, N = _prep(u)
+    _check(lib().oracle_fft2(_dptr(a), N, int(sign)), "fft2")
+    return a
+
+
+def fftshift(u):
+    a, N = _prep(u)
+    _check(lib().oracle_fftshift(_dptr(a), N), "fftshift")
+    return a
+
+
+def ifftshift(u):
+    a, N = _prep(u)
+    _check(lib().oracle_ifftshift(_dptr(a), N), "ifftshift")
+    return a
+
+
+def fft2d(u, direction, centered):
+    a, N = _prep(u)
+    _check(lib().oracle_fft2d(_dptr(a), N, int(direction), int(bool(centered))), "fft2d")
+    return a
+
+
+def apply_qpf(u, dx, lam, z):
+    a, N = _prep(u)
+    _check(lib().oracle_apply_qpf(_dptr(a), N, float(dx), float(lam), float(z)), "apply_qpf")
+    return a
+
+
+def apply_mask(u, amp, opd, lam):
+    a, N = _prep(u)
+    ka, pa = _real(amp, N)
+    ko, po = _real(opd, N)
+    _check(lib().oracle_apply_mask(_dptr(a), N, pa, po, float(lam)), "apply_mask")
+    return a
+
+
+def propagate_as(u, dx, lam, z):
+    a, N = _prep(u)
+    _check(lib().oracle_propagate_as(_dptr(a), N, float(dx), float(lam), float(z)), "propagate_as")
+    return a
+
+
+def propagate_direct(u, dx, lam, z):
+    """Returns (field, dx_out)."""
+    a, N = _prep(u)
+    d = ctypes.c_double(float(dx))
+    _check(lib().oracle_propagate_direct(_dptr(a), N, ctypes.byref(d), float(lam), float(z)), "propagate_direct")
+    return a, d.value
+
+
+def surface_as(u, dx, lam, f, amp, opd, z):
+    a, N = _prep(u)
+    ka, pa = _real(amp, N)
+    ko, po = _real(opd, N)
+    _check(lib().oracle_surface_as(_dptr(a), N, float(dx), float(lam),
+                                   float(f) if f is not None else math.inf, pa, po, float(z)), "surface_as")
+    return a
+
+
+# -- batch helpers: the batch dimension is just a loop over independent wavefronts --
+
+def _per_batch(x, b):
+    arr = np.atleast_1d(np.asarray(x, dtype=np.float64))
+    return float(arr[b] if arr.size > 1 else arr[0])
+
+
+def propagate_as_batch(u, dx, lam, z):
+    u = np.asarray(u)
+    return np.stack([propagate_as(u[b], _per_batch(dx, b), _per_batch(lam, b), z) for b in range(u.shape[0])])
+
+
+def surface_as_batch(u, dx, lam, f, amp, opd, z):
+    u = np.asarray(u)
+    return np.stack([surface_as(u[b], _per_batch(dx, b), _per_batch(lam, b), f, amp, opd, z)
+                     for b in range(u.shape[0])])

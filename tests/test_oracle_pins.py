@@ -1,0 +1,376 @@
+"""Pins for the CPU oracle (DESIGN.md "Oracle pins" P0..P13): closed forms, exact identities, brute
+force and the paper's own worked example.  Nothing here touches the GPU or the CUDA library.
+
+Each pin is chosen so that a plausible mistake in oracle/fresnel_oracle.c (a dropped term, a wrong
+sign or index, a transposed operand, a wrong scale) fails at least one of them.
+"""
+import math
+import os
+
+import numpy as np
+import pytest
+from scipy.special import j1
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+PI_L = 4 * np.arctan(np.longdouble(1))      # pi to long-double precision (np.pi is only a double)
+
+
+def rel(a, b):
+    return float(np.linalg.norm(a - b) / np.linalg.norm(b))
+
+
+def rnd(N, seed):
+    r = np.random.Generator(np.random.PCG64(seed))
+    return r.standard_normal((N, N)) + 1j * r.standard_normal((N, N))
+
+
+def coords(N, dx):
+    c = (np.arange(N) - N // 2) * dx
+    return c[None, :], c[:, None]     # x (varies along k, the fast axis), y (along j)
+
+
+# ---------------------------------------------------------------- P0 / definition of the DFT itself
+def test_dft2_naive_closed_forms(oracle):
+    """The brute-force DFT against closed forms: a delta transforms to a constant, a single complex
+    exponential exp(+2 pi i (j p0 + k q0)/N) transforms (forward kernel exp(-...)) to N^2 at
+    [p0, q0] -- pins sign, axis order and scaling of the definition everything else rests on."""
+    N = 16
+    d = np.zeros((N, N), complex)
+    d[0, 0] = 1.0
+    assert np.allclose(oracle.dft2_naive(d, -1), 1.0, atol=1e-15)
+    p0, q0 = 3, 5
+    j, k = np.meshgrid(np.arange(N), np.arange(N), indexing="ij")
+    e = np.exp(2j * np.pi * (j * p0 + k * q0) / N)
+    F = oracle.dft2_naive(e, -1)
+    expect = np.zeros((N, N), complex)
+    expect[p0, q0] = N * N
+    assert np.abs(F - expect).max() < 1e-11
+    # inverse kernel: same input lands at [-p0, -q0] with scale 1/N^2 ... and e itself maps from a delta
+    G = oracle.dft2_naive(expect, +1)
+    assert np.abs(G - e).max() < 1e-13
+    # a shifted delta gives the conjugate-phase ramp: F[p,q] = exp(-2 pi i (p j0 + q k0)/N)
+    d = np.zeros((N, N), complex)
+    d[2, 7] = 1.0
+    F = oracle.dft2_naive(d, -1)
+    assert np.abs(F - np.exp(-2j * np.pi * (j * 2 + k * 7) / N)).max() < 1e-14
+
+
+@pytest.mark.parametrize("N", [8, 16, 32, 64])
+@pytest.mark.parametrize("sign", [-1, +1])
+def test_P0_fft2_vs_bruteforce(oracle, N, sign):
+    u = rnd(N, 10 + N)
+    assert rel(oracle.fft2(u, sign), oracle.dft2_naive(u, sign)) <= 1e-13
+
+
+def test_fft2_reduces_to_library_routine(oracle):
+    u = rnd(512, 77)
+    assert rel(oracle.fft2(u, -1), np.fft.fft2(u)) <= 1e-14
+    assert rel(oracle.fft2(u, +1), np.fft.ifft2(u)) <= 1e-14
+
+
+# ---------------------------------------------------------------- P1 round trip
+def test_P1_round_trip(oracle):
+    u = rnd(256, 1)
+    assert rel(oracle.fft2(oracle.fft2(u, -1), +1), u) <= 1e-14
+    assert rel(oracle.fft2d(oracle.fft2d(u, oracle.FORWARD, 1), oracle.INVERSE, 1), u) <= 1e-14
+
+
+# ---------------------------------------------------------------- P2 inverse pairs
+def test_P2_inverse_pairs(oracle):
+    N, dx, lam, z = 1024, 2e-5, 1e-6, 0.7
+    u = rnd(N, 2)
+    assert rel(oracle.propagate_as(oracle.propagate_as(u, dx, lam, z), dx, lam, -z), u) <= 1e-13
+    assert rel(oracle.apply_qpf(oracle.apply_qpf(u, dx, lam, z), dx, lam, -z), u) <= 1e-14
+    v, dx1 = oracle.propagate_direct(u, dx, lam, z)
+    assert dx1 == pytest.approx(lam * z / (N * dx), rel=1e-15)
+    w, dx2 = oracle.propagate_direct(v, dx1, lam, -z)
+    assert dx2 == pytest.approx(dx, rel=1e-14)
+    # dx2 equals dx only to one rounding (dx1 is a rounded double); the ~1e3 rad corner phase of the
+    # last chirp turns that 1e-16 relative pitch error into ~1e-13 of field error.
+    assert rel(w, u) <= 1e-12
+
+
+# ---------------------------------------------------------------- P3 Parseval
+def test_P3_parseval(oracle):
+    N, dx, lam, z = 512, 2e-5, 0.8e-6, 0.3
+    u = rnd(N, 3)
+    e0 = np.sum(np.abs(u) ** 2)
+    v = oracle.propagate_as(u, dx, lam, z)
+    assert np.sum(np.abs(v) ** 2) / e0 == pytest.approx(1.0, abs=1e-13)
+    w, dx1 = oracle.propagate_direct(u, dx, lam, z)
+    assert np.sum(np.abs(w) ** 2) * dx1 ** 2 / (e0 * dx ** 2) == pytest.approx(1.0, abs=1e-13)
+    F = oracle.fft2(u, -1)
+    assert np.sum(np.abs(F) ** 2) / (N * N * e0) == pytest.approx(1.0, abs=1e-13)
+
+
+# ---------------------------------------------------------------- P4 Gaussian beam closed form
+def gaussian_closed_form(N, dx, lam, w0, z):
+    """U(r, z) = (q0/q) exp(i pi r^2/(lam q)), q0 = -i zR, q = q0 + z, zR = pi w0^2/lam
+    (textbook Gaussian beam: w(z) = w0 sqrt(1+(z/zR)^2), on-axis amplitude w0/w, Gouy phase
+    -atan(z/zR), curvature R = z (1+(zR/z)^2)); no piston exp(ikz) (reading g5)."""
+    x, y = coords(N, dx)
+    zR = math.pi * w0 * w0 / lam
+    q0 = -1j * zR
+    q = q0 + z
+    return (q0 / q) * np.exp(1j * np.pi * (x * x + y * y) / (lam * q))
+
+
+def test_P4_gaussian_beam_as(oracle):
+    N, dx, lam, w0 = 1024, 2e-5, 1.064e-6, 2e-3
+    u0 = gaussian_closed_form(N, dx, lam, w0, 0.0)
+    assert np.abs(u0.imag).max() < 1e-15 and u0[N // 2, N // 2].real == pytest.approx(1.0)
+    for z, tol in [(0.5, 1e-9), (2.0, 1e-9), (5.0, 1e-8)]:
+        v = oracle.propagate_as(u0, dx, lam, z)
+        assert rel(v, gaussian_closed_form(N, dx, lam, w0, z)) <= tol
+    # the physics the north star names: w(z) = w0 sqrt(1 + (z/zR)^2) from the second moment
+    z = 5.0
+    v = oracle.propagate_as(u0, dx, lam, z)
+    x, y = coords(N, dx)
+    I = np.abs(v) ** 2
+    w_num = math.sqrt(2.0 * np.sum(I * (x * x + y * y)) / np.sum(I))
+    zR = math.pi * w0 * w0 / lam
+    assert w_num == pytest.approx(w0 * math.sqrt(1 + (z / zR) ** 2), rel=1e-6)
+    assert abs(v[N // 2, N // 2]) == pytest.approx(1 / math.sqrt(1 + (z / zR) ** 2), rel=1e-9)
+    assert np.angle(v[N // 2, N // 2]) == pytest.approx(-math.atan(z / zR), abs=1e-9)
+
+
+@pytest.mark.parametrize("z", [0.5, 2.0, 5.0, -0.5])
+def test_P4_gaussian_beam_direct(oracle, z):
+    N, dx, lam, w0 = 1024, 2e-5, 1.064e-6, 2e-3
+    u0 = gaussian_closed_form(N, dx, lam, w0, 0.0)
+    v, dx1 = oracle.propagate_direct(u0, dx, lam, z)
+    assert dx1 == pytest.approx(lam * abs(z) / (N * dx), rel=1e-15)
+    if z == 0.5:
+        assert dx1 == pytest.approx(2.598e-5, rel=2e-4)
+    assert rel(v, gaussian_closed_form(N, dx1, lam, w0, z)) <= 1e-9
+
+
+# ---------------------------------------------------------------- P5 Gaussian through lenses (config 2)
+def abcd_chain(lam, w0, steps):
+    """Complex beam parameter through thin lenses and free space:
+    lens: 1/q <- 1/q - 1/f;  free space z: A <- A q/(q+z), q <- q+z;  field A exp(i pi r^2/(lam q))."""
+    q = -1j * math.pi * w0 * w0 / lam
+    A = 1.0 + 0j
+    out = []
+    for f, z in steps:
+        q = 1.0 / (1.0 / q - 1.0 / f)
+        A = A * q / (q + z)
+        q = q + z
+        out.append((q, A))
+    return out
+
+
+def test_P5_gaussian_lens_chain(oracle):
+    from paper_1806_06467_b200 import inputs
+    wl = inputs.config2()
+    N, dx, lam, w0 = wl.N, float(wl.dx[0]), float(wl.lam[0]), 2e-3
+    steps = [(s.f, s.z) for s in wl.surfaces]
+    ref = abcd_chain(lam, w0, steps)
+    # beam parameters after each stage (values recorded in SURVEY.md sec. 8(c) P5)
+    w = [math.sqrt(lam / (math.pi * (1 / q).imag)) for q, _ in ref]
+    assert w[0] == pytest.approx(84.67e-6, rel=1e-3)
+    assert w[1] == pytest.approx(3.0003e-3, rel=1e-4)
+    assert w[2] == pytest.approx(4.0036e-3, rel=1e-4)
+    assert [abs(A) for _, A in ref] == pytest.approx([23.621, 0.6666, 0.49955], rel=2e-4)
+
+    # direct chain: pixel scale changes at every step
+    u, d = wl.field[0], dx
+    tol_direct = [1e-8, 1e-8, 1e-8]
+    for (f, z), (q, A), tol in zip(steps, ref, tol_direct):
+        u = oracle.apply_qpf(u, d, lam, -f)
+        u, d = oracle.propagate_direct(u, d, lam, z)
+        x, y = coords(N, d)
+        assert rel(u, A * np.exp(1j * np.pi * (x * x + y * y) / (lam * q))) <= tol
+        I = np.abs(u) ** 2
+        w_num = math.sqrt(2.0 * np.sum(I * (x * x + y * y)) / np.sum(I))
+        assert w_num == pytest.approx(math.sqrt(lam / (math.pi * (1 / q).imag)), rel=1e-5)
+    assert d == pytest.approx(3.464e-5, rel=2e-4)
+
+    # angular-spectrum chain: fixed pixel scale; the beam reaches the grid edge at stages 2 and 3
+    # (half-width/w = 3.4 then 2.6), so those tolerances are grid truncation, not oracle error.
+    u = wl.field[0]
+    x, y = coords(N, dx)
+    for (f, z), (q, A), tol in zip(steps, ref, [1e-9, 1e-4, 5e-3]):
+        u = oracle.surface_as(u, dx, lam, f, None, None, z)
+        assert rel(u, A * np.exp(1j * np.pi * (x * x + y * y) / (lam * q))) <= tol
+
+
+# ---------------------------------------------------------------- P6 Talbot, exact
+def test_P6_talbot_exact(oracle):
+    N, dx, lam, dpx = 256, 1e-5, 1e-6, 16
+    cell = rnd(dpx, 6)
+    u = np.tile(cell, (N // dpx, N // dpx))
+    d = dpx * dx
+    zT = 2 * d * d / lam
+    assert rel(oracle.propagate_as(u, dx, lam, zT), u) <= 1e-13
+    half = oracle.propagate_as(u, dx, lam, zT / 2)
+    assert rel(half, np.roll(u, (dpx // 2, dpx // 2), axis=(0, 1))) <= 1e-13
+    assert rel(half, u) > 0.5      # and it is NOT the unshifted field
+
+
+# ---------------------------------------------------------------- P7 Talbot, the paper's example
+def read_golden(name):
+    out = {}
+    with open(os.path.join(HERE, "golden", name)) as fh:
+        for line in fh:
+            if line.strip() and not line.startswith("#"):
+                k, v = line.split()
+                out[k] = float(v)
+    return out
+
+
+def test_P7_talbot_paper_example(oracle):
+    g = read_golden("talbot_paper_example.txt")
+    lam = 1e-6                                             # reading g14
+    D, cyc, amp_m = g["aperture_diameter_m"], g["cycles_per_aperture"], g["wfe_amplitude_m"]
+    d = D / cyc                                            # grating period: 1 mm
+    ZT = 2 * (D / cyc) ** 2 / lam                          # Eq. 1
+    assert d == pytest.approx(1e-3) and ZT == pytest.approx(2.0)
+    N, dx = 256, d / 16
+    x, _ = coords(N, dx)
+    eps = 2 * math.pi * amp_m / lam
+    c = np.cos(2 * np.pi * x / d) * np.ones((N, 1))
+    u0 = np.exp(1j * eps * c)
+    # complete phase -> amplitude conversion at 0.25 Z_T
+    u = oracle.propagate_as(u0, dx, lam, g["full_conversion_zt"] * ZT)
+    a = np.abs(u)
+    coef = np.sum((a - a.mean()) * c) / np.sum(c * c) / eps
+    assert coef == pytest.approx(1.0, abs=5e-4)           # +eps*cos: the opposite sign of H gives -1
+    assert np.abs(a - (1 + eps * c)).max() <= 0.75 * eps * eps
+    ph = np.angle(u)
+    assert np.sqrt(np.mean((ph - ph.mean()) ** 2)) <= 1e-12   # phase is flat
+    # partial conversion at 0.05 Z_T: amplitude modulation eps*sin(2 pi z/Z_T), residual phase eps*cos(2 pi z/Z_T)
+    zf = g["partial_conversion_zt"]
+    u = oracle.propagate_as(u0, dx, lam, zf * ZT)
+    a = np.abs(u)
+    coef = np.sum((a - a.mean()) * c) / np.sum(c * c) / eps
+    assert coef == pytest.approx(math.sin(2 * math.pi * zf), abs=2e-3)
+    ph = np.angle(u)
+    pcoef = np.sum((ph - ph.mean()) * c) / np.sum(c * c) / eps
+    assert pcoef == pytest.approx(math.cos(2 * math.pi * zf), abs=2e-3)
+
+
+# ---------------------------------------------------------------- P8 Airy far field
+def test_P8_airy(oracle):
+    from paper_1806_06467_b200 import inputs
+    N, dx, lam, apx, f = 1024, 1e-5, 1e-6, 32, 0.5
+    ap = inputs.circular_aperture(N, apx).astype(complex)
+    u = oracle.apply_qpf(ap, dx, lam, -f)
+    v, dx1 = oracle.propagate_direct(u, dx, lam, f)
+    centre = v[N // 2, N // 2]
+    expect_centre = ap.sum().real * dx * dx / (1j * lam * f)
+    assert abs(centre - expect_centre) <= 1e-12 * abs(expect_centre)
+    assert centre.imag == pytest.approx(-0.6418, abs=2e-4) and abs(centre.real) < 1e-12
+    a = apx * dx
+    rp = (np.arange(N) - N // 2) * dx1
+    sl = slice(N // 2 - 60, N // 2 + 61)
+    vv = 2 * np.pi * a * np.abs(rp[sl]) / (lam * f)
+    with np.errstate(invalid="ignore", divide="ignore"):
+        airy = np.where(vv == 0, 1.0, 2 * j1(vv) / vv)
+    model = (np.pi * a * a / (lam * f)) * np.abs(airy)
+    peak = model.max()
+    assert np.abs(np.abs(v[N // 2, sl]) - model).max() <= 5e-3 * peak      # row cut
+    assert np.abs(np.abs(v[sl, N // 2]) - model).max() <= 5e-3 * peak      # column cut
+    prof = np.abs(v[N // 2, N // 2:N // 2 + 40])
+    first_min = int(np.argmax((prof[1:-1] < prof[:-2]) & (prof[1:-1] < prof[2:]))) + 1
+    assert abs(first_min - 0.6098 * N * dx / a) <= 1.0                      # 19.51 px predicted
+
+
+# ---------------------------------------------------------------- P9 AS == direct at the critical distance
+def test_P9_as_equals_direct_at_critical_distance(oracle):
+    N, dx, lam = 1024, 2e-5, 1e-6
+    zc = N * dx * dx / lam
+    x, y = coords(N, dx)
+    u = np.exp(-(x * x + y * y) / (2e-3) ** 2) * np.exp(0.1j * np.cos(2 * np.pi * x / (32 * dx)))
+    a = oracle.propagate_as(u, dx, lam, zc)
+    b, dx1 = oracle.propagate_direct(u, dx, lam, zc)
+    assert dx1 == pytest.approx(dx, rel=1e-14)
+    assert rel(a, b) <= 1e-12
+
+
+# ---------------------------------------------------------------- P10 semigroup
+def test_P10_semigroup(oracle):
+    N, dx, lam = 256, 1e-5, 1e-6
+    u = rnd(N, 10)
+    a = oracle.propagate_as(oracle.propagate_as(u, dx, lam, 0.013), dx, lam, 0.021)
+    assert rel(a, oracle.propagate_as(u, dx, lam, 0.034)) <= 1e-13
+    assert rel(oracle.propagate_as(u, dx, lam, 0.0), u) <= 1e-14          # z = 0 is the identity (g11)
+
+
+# ---------------------------------------------------------------- P11 shift bookkeeping
+def test_P11_shift_bookkeeping(oracle):
+    N, dx, lam, z = 256, 1e-5, 1e-6, 0.02
+    u = rnd(N, 11)
+    # literal shifted AS == unshifted AS with H in FFT order (same long-double phase evaluation)
+    m = np.where(np.arange(N) < N // 2, np.arange(N), np.arange(N) - N).astype(np.longdouble)
+    fq = m / (np.longdouble(N) * np.longdouble(dx))
+    th = -PI_L * np.longdouble(lam) * np.longdouble(z) * (fq[None, :] ** 2 + fq[:, None] ** 2)
+    H = np.cos(th).astype(np.float64) + 1j * np.sin(th).astype(np.float64)
+    unshifted = oracle.fft2(oracle.fft2(u, -1) * H, +1)
+    assert rel(unshifted, oracle.propagate_as(u, dx, lam, z)) <= 1e-15
+    # the rotations themselves
+    assert np.array_equal(oracle.fftshift(u), np.fft.fftshift(u))
+    assert np.array_equal(oracle.ifftshift(u), np.fft.ifftshift(u))
+    # centred FFT == s * fft2(s * u), s = (-1)^(j+k): exactly
+    j, k = np.meshgrid(np.arange(N), np.arange(N), indexing="ij")
+    s = (-1.0) ** (j + k)
+    assert np.array_equal(oracle.fft2d(u, oracle.FORWARD, 1), s * oracle.fft2(s * u, -1))
+    assert np.array_equal(oracle.fft2d(u, oracle.INVERSE, 1), s * oracle.fft2(s * u, +1))
+
+
+# ---------------------------------------------------------------- P12 QPF structure
+def test_P12_qpf_structure(oracle):
+    N, dx, lam, z = 512, 2e-5, 550e-9, -0.2          # lens f = 0.2 m: corner phase ~ 1.5e3 rad
+    Q = oracle.apply_qpf(np.ones((N, N), complex), dx, lam, z)
+    assert Q[N // 2, N // 2] == 1.0 + 0j
+    assert np.array_equal(Q[1:, :], Q[:0:-1, :]) and np.array_equal(Q[:, 1:], Q[:, :0:-1])
+    assert np.array_equal(Q, Q.T)
+    assert np.abs(np.abs(Q) - 1).max() < 1e-15
+    c = ((np.arange(N) - N // 2) * np.longdouble(dx))
+    th = PI_L * c * c / (np.longdouble(lam) * np.longdouble(z))
+    t = np.cos(th).astype(np.float64) + 1j * np.sin(th).astype(np.float64)
+    assert np.abs(Q - t[:, None] * t[None, :]).max() <= 1e-14
+    # sign and scale of the phase (reading g1): one pixel off axis the phase is pi dx^2/(lam z)
+    assert np.angle(Q[N // 2, N // 2 + 1]) == pytest.approx(math.pi * dx * dx / (lam * z), rel=1e-12)
+    # x runs along the fast axis, y along the slow one; the chirp is the same in both
+    assert Q[N // 2 + 3, N // 2] == Q[N // 2, N // 2 + 3]
+
+
+# ---------------------------------------------------------------- P13 mask special cases
+def test_P13_mask_special_cases(oracle):
+    N, lam = 128, 633e-9
+    u = rnd(N, 13)
+    assert np.array_equal(oracle.apply_mask(u, None, None, lam), u)
+    assert np.array_equal(oracle.apply_mask(u, np.ones((N, N)), np.zeros((N, N)), lam), u)
+    assert rel(oracle.apply_mask(u, None, np.full((N, N), lam), lam), u) <= 1e-15
+    A = (np.random.Generator(np.random.PCG64(5)).random((N, N)) < 0.5).astype(float)
+    v = oracle.apply_mask(u, A, None, lam)
+    assert np.all(v[A == 0] == 0) and np.array_equal(v[A == 1], u[A == 1])
+    # quarter-wave OPD multiplies by +i (sign of Eq. 3, reading g3)
+    w = oracle.apply_mask(u, None, np.full((N, N), lam / 4), lam)
+    assert rel(w, 1j * u) <= 1e-15
+    # non-uniform map, against the definition evaluated with numpy
+    opd = np.random.Generator(np.random.PCG64(6)).normal(0, 20e-9, (N, N))
+    assert rel(oracle.apply_mask(u, A, opd, lam), u * A * np.exp(2j * np.pi * opd / lam)) <= 1e-15
+
+
+def test_surface_as_is_the_literal_composition(oracle):
+    N, dx, lam = 256, 2e-5, 550e-9
+    u = rnd(N, 14)
+    r = np.random.Generator(np.random.PCG64(7))
+    A, opd = (r.random((N, N)) < 0.7).astype(float), r.normal(0, 10e-9, (N, N))
+    lit = oracle.propagate_as(oracle.apply_mask(oracle.apply_qpf(u, dx, lam, -0.8), A, opd, lam), dx, lam, 0.4)
+    assert np.array_equal(oracle.surface_as(u, dx, lam, 0.8, A, opd, 0.4), lit)
+    assert np.array_equal(oracle.surface_as(u, dx, lam, math.inf, None, None, 0.4), oracle.propagate_as(u, dx, lam, 0.4))
+
+
+def test_oracle_rejects_bad_arguments(oracle):
+    u = rnd(64, 15)
+    with pytest.raises(oracle.OracleError):
+        oracle.apply_qpf(u, 1e-5, 1e-6, 0.0)
+    with pytest.raises(oracle.OracleError):
+        oracle.propagate_direct(u, 1e-5, 1e-6, 0.0)
+    with pytest.raises(oracle.OracleError):
+        oracle.propagate_as(u, -1e-5, 1e-6, 0.1)
+    with pytest.raises(oracle.OracleError):
+        oracle.dft2_naive(rnd(128, 1), -1)

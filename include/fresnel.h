@@ -1,0 +1,135 @@
+/*
+ * fresnel.h -- C ABI of libfresnel.so: B200-native plane-to-plane Fresnel propagation.
+ *
+ * The hot path of arXiv 1806.06467 (Douglas & Perrin, "Accelerated Modeling of Near and Far-Field
+ * Diffraction for Coronagraphic Optical Systems"): a complex N x N wavefront multiplied by quadratic
+ * phase factors (thin lenses, Fresnel chirps), 2-D forward/inverse FFTs and the angular-spectrum
+ * transfer function, surface after surface (BASELINE.json:north_star).
+ * Citations "PAPER.md:L" are line numbers of /root/reference/PAPER.md; "gK" are the readings listed
+ * in DESIGN.md where the paper is silent or garbled.
+ *
+ * CONVENTIONS (all entry points)
+ *   Wavefront  `wf`: DEVICE pointer, row-major [batch][N][N], interleaved (re, im) of the plan's
+ *              dtype (float2 for FRESNEL_C64, double2 for FRESNEL_C128), 16-byte aligned, modified
+ *              IN PLACE.  The caller owns it.  Pixel [j][k] sits at y = (j - N/2)*dx, x = (k - N/2)*dx
+ *              (origin on pixel N/2: the fftshift convention of PAPER.md:123, reading g8).
+ *   pixel, lambda: HOST arrays of length `batch` (metres): pixel pitch dx_b and wavelength of every
+ *              batch element ("repeated for all of the wavelengths").  They are consumed
+ *              before the call returns.
+ *   amp, opd:  DEVICE pointers to real [N][N] maps of matching precision (float / double), shared
+ *              by the whole batch; either may be NULL.  The caller owns them.
+ *   Execution: every call only ENQUEUES work on the plan's CUDA stream and returns without
+ *              synchronising (except fresnel_plan_synchronize and plan create/destroy).  No device
+ *              memory is allocated in the hot calls: the plan owns FFT twiddles, chirp tables and
+ *              per-batch scalars.  All hot calls are CUDA-graph capturable.
+ *   Errors:    return codes only, never exceptions or aborts.  On any error nothing is enqueued.
+ *                FRESNEL_ERR_INVALID_ARG  NULL plan/wf/host array, lambda <= 0, pixel <= 0, non-finite
+ *                                         z, z == 0 where a division by z is needed, f == 0 or NaN,
+ *                                         bad direction
+ *                FRESNEL_ERR_UNSUPPORTED  N not a power of two in [64, 8192] (the paper's N = 2800
+ *                                         run, is a later milestone), bad dtype
+ *                FRESNEL_ERR_ALLOC        device/host allocation failed (plan create only)
+ *                FRESNEL_ERR_CUDA         a CUDA runtime call or launch failed
+ *   Threads:   a plan is not thread-safe; distinct plans are independent.
+ *   There is no CPU fallback: without a CUDA device plan creation fails with FRESNEL_ERR_CUDA.
+ */
+#ifndef FRESNEL_H
+#define FRESNEL_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct fresnel_plan fresnel_plan; /* opaque */
+
+typedef enum { FRESNEL_C64 = 0, FRESNEL_C128 = 1 } fresnel_dtype;
+
+typedef enum {
+    FRESNEL_OK = 0,
+    FRESNEL_ERR_INVALID_ARG = 1,
+    FRESNEL_ERR_UNSUPPORTED = 2,
+    FRESNEL_ERR_ALLOC = 3,
+    FRESNEL_ERR_CUDA = 4
+} fresnel_status;
+
+enum { FRESNEL_FORWARD = +1, FRESNEL_INVERSE = -1 };
+
+/* ---- plan ------------------------------------------------------------------------------------ */
+
+/* Create a plan for `batch` wavefronts of N x N complex elements of `dtype` on the current CUDA
+ * device.  Builds the FFT twiddle tables (host long double, rounded once) and allocates the chirp
+ * table cache.  N: power of two in [64, 8192]; batch >= 1.  *out is set only on FRESNEL_OK. */
+fresnel_status fresnel_plan_create(fresnel_plan **out, int N, int batch, fresnel_dtype dtype);
+
+/* Stream all later calls enqueue on (a cudaStream_t passed as void*; NULL = legacy default stream). */
+fresnel_status fresnel_plan_set_stream(fresnel_plan *p, void *cuda_stream);
+
+/* Block the host until everything enqueued on the plan's stream has finished. */
+fresnel_status fresnel_plan_synchronize(fresnel_plan *p);
+
+/* Synchronises the plan's stream, frees everything the plan owns.  NULL is a no-op. */
+fresnel_status fresnel_plan_destroy(fresnel_plan *p);
+
+/* Number of kernels this plan has launched so far (bench.py reports it as gpu_launches). */
+fresnel_status fresnel_plan_launch_count(const fresnel_plan *p, unsigned long long *count);
+
+/* ---- the operations of the hot path ----------------------------------------------------------- */
+
+/* Quadratic phase factor, Eq. 2 read as (g1)
+ *     wf[b][j][k] *= exp(+i*pi*(x_k^2 + y_j^2) / (lambda_b * z)),   x, y from pixel[b].
+ * A thin lens of focal length f (PAPER.md:29 "treated as thin lenses", :239-244 QuadraticLens) is
+ * z = -f (converging for f > 0, reading g2).  z == 0 or non-finite: FRESNEL_ERR_INVALID_ARG.
+ * One pass over the wavefront; the chirp is applied as the outer product of one 1-D table. */
+fresnel_status fresnel_apply_qpf(fresnel_plan *p, void *wf, const double *pixel, const double *lambda, double z);
+
+/* Optic phasor, Eq. 3:  wf[b][j][k] *= amp[j][k] * exp(2*pi*i*opd[j][k]/lambda_b),
+ * opd in metres, sign + (reading g3).  amp == NULL means 1, opd == NULL means 0; both NULL is a no-op. */
+fresnel_status fresnel_apply_mask(fresnel_plan *p, void *wf, const void *amp, const void *opd, const double *lambda);
+
+/* 2-D FFT (bottleneck #1).  direction = FRESNEL_FORWARD: unnormalised, kernel
+ * exp(-2*pi*i*(j*p + k*q)/N);  FRESNEL_INVERSE: kernel exp(+...), scaled by 1/N^2 (reading g6).
+ * centered != 0 computes fftshift(fft2(ifftshift(wf))) with zero extra memory
+ * passes: for even N it equals s*fft2(s*wf), s = (-1)^(j+k), applied on load and on store. */
+fresnel_status fresnel_fft2d(fresnel_plan *p, void *wf, int direction, int centered);
+
+/* Angular-spectrum plane-to-plane propagation by z (BASELINE.json:north_star):
+ *     wf <- fftshift(ifft2( fft2(ifftshift(wf)) * H )),   H = exp(-i*pi*lambda*z*(fx^2 + fy^2)),
+ * fx, fy = FFT-order frequencies q/(N*dx).  No piston exp(ikz) (g5); unit gain; pixel pitch unchanged;
+ * z < 0 allowed (g10); z == 0 is the identity (g11).  Because H = Hx (x) Hy is separable the
+ * operator is a row convolution followed by a column convolution: TWO passes over the wavefront,
+ * each doing FFT -> x H1 -> inverse FFT on chip; the shifts cancel exactly and cost nothing. */
+fresnel_status fresnel_propagate_as(fresnel_plan *p, void *wf, const double *pixel, const double *lambda, double z);
+
+/* Direct (single-FFT) Fresnel propagation by z != 0 (PAPER.md:29 "direct Fresnel", :53 pixelscale):
+ *     wf <- (dx^2/(i*lambda*z)) * Q_dx'(z) * CFT( Q_dx(z) * wf ),    dx' = lambda*|z|/(N*dx),
+ * Q_d(z) the chirp of fresnel_apply_qpf at pitch d, CFT the centred transform with the forward
+ * kernel for z > 0 and the unnormalised inverse kernel for z < 0 (readings g7, g10).
+ * pixel_inout (HOST, length batch) is read as dx and overwritten with dx' before the call returns. */
+fresnel_status fresnel_propagate_direct(fresnel_plan *p, void *wf, double *pixel_inout, const double *lambda, double z);
+
+/* One whole surface, fused ("add_optic(optic, distance=...)"):
+ *     apply_qpf(z = -f)  [skipped if f is +-INFINITY]  ->  apply_mask(amp, opd)  ->  propagate_as(z)
+ * in the same two passes as fresnel_propagate_as: the optic phasor and the x-chirp of the lens ride on
+ * the load of the row pass, the y-chirp on the load of the column pass.  z == 0: optic only. */
+fresnel_status fresnel_surface_as(fresnel_plan *p, void *wf, const double *pixel, const double *lambda,
+                                  double f, const void *amp, const void *opd, double z);
+
+/* ---- host <-> device staging on the plan's stream (used by the end-to-end benchmark) ---------- */
+
+/* Asynchronous copies ordered with the plan's work.  `host` should be pinned for real overlap. */
+fresnel_status fresnel_memcpy_h2d(fresnel_plan *p, void *dst_device, const void *src_host, size_t bytes);
+fresnel_status fresnel_memcpy_d2h(fresnel_plan *p, void *dst_host, const void *src_device, size_t bytes);
+
+/* ---- misc -------------------------------------------------------------------------------------- */
+
+const char *fresnel_status_string(fresnel_status s);
+
+/* Library build string, e.g. "fresnel-b200 0.1 sm_100a". */
+const char *fresnel_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FRESNEL_H */

@@ -1,0 +1,200 @@
+"""Thin ctypes face of libfresnel.so (the C ABI declared in include/fresnel.h).
+
+Argument marshalling only: every step of the path runs in the library's CUDA kernels.  torch is
+used for device memory and streams, nothing else.  There is NO fallback: if libfresnel.so is
+missing or a call fails, an exception is raised.
+
+    plan = Plan(N=2048, batch=1, dtype="c128")
+    plan.surface_as(wf, pixel=[2e-5], lam=[550e-9], f=0.5, amp=amp, opd=opd, z=0.3)   # in place
+"""
+from __future__ import annotations
+
+import ctypes
+import math
+import os
+from typing import Optional, Sequence
+
+import numpy as np
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libfresnel.so")
+
+FRESNEL_OK = 0
+FORWARD = +1
+INVERSE = -1
+C64, C128 = 0, 1
+
+# every symbol include/fresnel.h declares (tests/test_abi.py checks the header against this list)
+SYMBOLS = (
+    "fresnel_plan_create", "fresnel_plan_set_stream", "fresnel_plan_synchronize", "fresnel_plan_destroy",
+    "fresnel_plan_launch_count", "fresnel_apply_qpf", "fresnel_apply_mask", "fresnel_fft2d",
+    "fresnel_propagate_as", "fresnel_propagate_direct", "fresnel_surface_as", "fresnel_memcpy_h2d",
+    "fresnel_memcpy_d2h", "fresnel_status_string", "fresnel_version",
+)
+
+_lib = None
+
+
+class FresnelError(RuntimeError):
+    def __init__(self, status: int, what: str):
+        self.status = status
+        name = lib().fresnel_status_string(status).decode() if _lib is not None else str(status)
+        super().__init__(f"{what}: {name}")
+
+
+def lib() -> ctypes.CDLL:
+    """Load libfresnel.so; fails loudly when the CUDA extension has not been built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise RuntimeError(f"{LIB_PATH} is missing: build it with `python -m paper_1806_06467_b200.build` "
+                           "(there is no CPU fallback)")
+    L = ctypes.CDLL(LIB_PATH)
+    vp, dp, ci, cd = ctypes.c_void_p, ctypes.POINTER(ctypes.c_double), ctypes.c_int, ctypes.c_double
+    L.fresnel_plan_create.argtypes = [ctypes.POINTER(vp), ci, ci, ci]
+    L.fresnel_plan_set_stream.argtypes = [vp, vp]
+    L.fresnel_plan_synchronize.argtypes = [vp]
+    L.fresnel_plan_destroy.argtypes = [vp]
+    L.fresnel_plan_launch_count.argtypes = [vp, ctypes.POINTER(ctypes.c_ulonglong)]
+    L.fresnel_apply_qpf.argtypes = [vp, vp, dp, dp, cd]
+    L.fresnel_apply_mask.argtypes = [vp, vp, vp, vp, dp]
+    L.fresnel_fft2d.argtypes = [vp, vp, ci, ci]
+    L.fresnel_propagate_as.argtypes = [vp, vp, dp, dp, cd]
+    L.fresnel_propagate_direct.argtypes = [vp, vp, dp, dp, cd]
+    L.fresnel_surface_as.argtypes = [vp, vp, dp, dp, cd, vp, vp, cd]
+    L.fresnel_memcpy_h2d.argtypes = [vp, vp, vp, ctypes.c_size_t]
+    L.fresnel_memcpy_d2h.argtypes = [vp, vp, vp, ctypes.c_size_t]
+    for s in SYMBOLS:
+        getattr(L, s).restype = ci
+    L.fresnel_status_string.argtypes = [ci]
+    L.fresnel_status_string.restype = ctypes.c_char_p
+    L.fresnel_version.argtypes = []
+    L.fresnel_version.restype = ctypes.c_char_p
+    _lib = L
+    return L
+
+
+def version() -> str:
+    return lib().fresnel_version().decode()
+
+
+def _darr(x, n: int):
+    a = np.ascontiguousarray(np.broadcast_to(np.asarray(x, dtype=np.float64), (n,)))
+    return a, a.ctypes.data_as(ctypes.POINTER(ctypes.c_double))
+
+
+class Plan:
+    """A fresnel_plan: N x N grids, `batch` wavefronts, dtype "c64" or "c128"."""
+
+    def __init__(self, N: int, batch: int = 1, dtype: str = "c128", stream=None):
+        import torch
+        self._torch = torch
+        self.N, self.batch, self.dtype = int(N), int(batch), dtype
+        code = {"c64": C64, "c128": C128}.get(dtype)
+        if code is None:
+            raise ValueError("dtype must be 'c64' or 'c128'")
+        self.cdtype = torch.complex64 if dtype == "c64" else torch.complex128
+        self.rdtype = torch.float32 if dtype == "c64" else torch.float64
+        self._h = ctypes.c_void_p()
+        st = lib().fresnel_plan_create(ctypes.byref(self._h), self.N, self.batch, code)
+        if st != FRESNEL_OK:
+            self._h = ctypes.c_void_p()
+            raise FresnelError(st, "fresnel_plan_create")
+        if stream is None:
+            stream = torch.cuda.current_stream()
+        self.set_stream(stream)
+
+    # -- plumbing ------------------------------------------------------------------------------
+    def set_stream(self, stream) -> None:
+        self._stream = stream
+        self._chk(lib().fresnel_plan_set_stream(self._h, ctypes.c_void_p(stream.cuda_stream)), "fresnel_plan_set_stream")
+
+    def synchronize(self) -> None:
+        self._chk(lib().fresnel_plan_synchronize(self._h), "fresnel_plan_synchronize")
+
+    def launch_count(self) -> int:
+        c = ctypes.c_ulonglong(0)
+        self._chk(lib().fresnel_plan_launch_count(self._h, ctypes.byref(c)), "fresnel_plan_launch_count")
+        return int(c.value)
+
+    def close(self) -> None:
+        if getattr(self, "_h", None) is not None and self._h.value:
+            lib().fresnel_plan_destroy(self._h)
+            self._h = ctypes.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _chk(self, st: int, what: str) -> None:
+        if st != FRESNEL_OK:
+            raise FresnelError(st, what)
+
+    def _wf(self, wf) -> ctypes.c_void_p:
+        if wf.dtype != self.cdtype or not wf.is_cuda or not wf.is_contiguous():
+            raise ValueError(f"wavefront must be a contiguous CUDA tensor of {self.cdtype}")
+        if wf.numel() != self.batch * self.N * self.N:
+            raise ValueError("wavefront must have batch*N*N elements")
+        return ctypes.c_void_p(wf.data_ptr())
+
+    def _map(self, m) -> ctypes.c_void_p:
+        if m is None:
+            return ctypes.c_void_p(None)
+        if m.dtype != self.rdtype or not m.is_cuda or not m.is_contiguous() or m.numel() != self.N * self.N:
+            raise ValueError(f"maps must be contiguous CUDA tensors of {self.rdtype} with N*N elements")
+        return ctypes.c_void_p(m.data_ptr())
+
+    # -- the C ABI, same names -------------------------------------------------------------------
+    def apply_qpf(self, wf, pixel, lam, z: float) -> None:
+        _, pp = _darr(pixel, self.batch)
+        _, lp = _darr(lam, self.batch)
+        self._chk(lib().fresnel_apply_qpf(self._h, self._wf(wf), pp, lp, float(z)), "fresnel_apply_qpf")
+
+    def apply_mask(self, wf, amp, opd, lam) -> None:
+        _, lp = _darr(lam, self.batch)
+        self._chk(lib().fresnel_apply_mask(self._h, self._wf(wf), self._map(amp), self._map(opd), lp), "fresnel_apply_mask")
+
+    def fft2d(self, wf, direction: int = FORWARD, centered: bool = False) -> None:
+        self._chk(lib().fresnel_fft2d(self._h, self._wf(wf), int(direction), int(bool(centered))), "fresnel_fft2d")
+
+    def propagate_as(self, wf, pixel, lam, z: float) -> None:
+        _, pp = _darr(pixel, self.batch)
+        _, lp = _darr(lam, self.batch)
+        self._chk(lib().fresnel_propagate_as(self._h, self._wf(wf), pp, lp, float(z)), "fresnel_propagate_as")
+
+    def propagate_direct(self, wf, pixel, lam, z: float) -> np.ndarray:
+        """Returns the new pixel pitch per batch element."""
+        pa, pp = _darr(pixel, self.batch)
+        pa = pa.copy()
+        pp = pa.ctypes.data_as(ctypes.POINTER(ctypes.c_double))
+        _, lp = _darr(lam, self.batch)
+        self._chk(lib().fresnel_propagate_direct(self._h, self._wf(wf), pp, lp, float(z)), "fresnel_propagate_direct")
+        return pa
+
+    def surface_as(self, wf, pixel, lam, f: Optional[float], amp, opd, z: float) -> None:
+        _, pp = _darr(pixel, self.batch)
+        _, lp = _darr(lam, self.batch)
+        ff = math.inf if f is None else float(f)
+        self._chk(lib().fresnel_surface_as(self._h, self._wf(wf), pp, lp, ff, self._map(amp), self._map(opd), float(z)),
+                  "fresnel_surface_as")
+
+    def memcpy_h2d(self, dst, src_host) -> None:
+        nbytes = src_host.numel() * src_host.element_size()
+        self._chk(lib().fresnel_memcpy_h2d(self._h, ctypes.c_void_p(dst.data_ptr()), ctypes.c_void_p(src_host.data_ptr()), nbytes),
+                  "fresnel_memcpy_h2d")
+
+    def memcpy_d2h(self, dst_host, src) -> None:
+        nbytes = src.numel() * src.element_size()
+        self._chk(lib().fresnel_memcpy_d2h(self._h, ctypes.c_void_p(dst_host.data_ptr()), ctypes.c_void_p(src.data_ptr()), nbytes),
+                  "fresnel_memcpy_d2h")
+
+
+def run_surfaces(plan: Plan, wf, pixel, lam, surfaces: Sequence, maps=None) -> None:
+    """Chain of fused surfaces ("10 optics ... 19 FFT"): one fresnel_surface_as per
+    surface.  `maps[i]` = (amp, opd) device tensors or None for surface i."""
+    for i, s in enumerate(surfaces):
+        amp, opd = (maps[i] if maps is not None else (None, None))
+        plan.surface_as(wf, pixel, lam, s.f, amp, opd, s.z)

@@ -1,0 +1,148 @@
+// pass_kernel.cuh -- ONE HBM round trip of the Fresnel hot path.
+//
+// A pass reads every line (row or column) of a [batch][N][N] wavefront once, and on chip does
+//     [optic phasor A*exp(2 pi i OPD/lambda)]  (row pass only; Eq. 3)
+//  -> [x pre[n]]                                (1-D chirp table: lens / Fresnel QPF, Eq. 2)
+//  -> FFT (MODE_FWD, MODE_CONV) or inverse FFT (MODE_INV)
+//  -> [x mid[k]]                                (transfer function H1 / output chirp / 1/N / signs)
+//  -> inverse FFT                               (MODE_CONV only)
+//  -> [x scale]
+// and writes the line back in place.  Angular-spectrum propagation is MODE_CONV over rows then
+// over columns (H is separable); fft2d and direct Fresnel are MODE_FWD/MODE_INV over rows then
+// columns.  Shifts are folded into the tables ((-1)^n signs) and never touch memory.
+#pragma once
+#include "fft_core.cuh"
+
+namespace fresnel {
+
+enum PassMode { MODE_FWD = 0, MODE_INV = 1, MODE_CONV = 2 };
+
+template <typename T> struct PassArgs {
+    using C = typename cplx_of<T>::type;
+    C *wf;                    // [batch][N][N]
+    const C *pre;             // [batch][N] or nullptr
+    const C *mid;             // [batch][N] or nullptr
+    const C *tw;              // FFT twiddle tables of this N
+    const T *amp;             // [N][N] or nullptr (row pass only)
+    const T *opd;             // [N][N] or nullptr (row pass only)
+    const double *inv_lambda; // [batch] 1/lambda (only read when opd != nullptr)
+    T scale;                  // applied last when != 1
+};
+
+// exp(2 pi i u) for a phase u given in turns (optic phasor; |u| is typically << 1)
+FR_DEV double2 phasor_turns(double u)
+{
+    double s, c;
+    sincospi(2.0 * u, &s, &c);
+    return make_double2(c, s);
+}
+FR_DEV float2 phasor_turns(float u)
+{
+    float s, c;
+    sincospif(2.0f * u, &s, &c);
+    return make_float2(c, s);
+}
+
+template <typename T, int N, bool COL, int W, int MODE, int MINB>
+__global__ void __launch_bounds__(W *(N / 16), MINB) pass_kernel(PassArgs<T> a)
+{
+    using C = typename cplx_of<T>::type;
+    constexpr int TL = N / 16;
+    extern __shared__ __align__(16) unsigned char fr_smem[];
+    C *buf = reinterpret_cast<C *>(fr_smem);
+
+    const int tid = threadIdx.x;
+    const int line = COL ? tid % W : tid / TL;
+    const int j = COL ? tid / W : tid % TL;
+    const int b = blockIdx.y;
+    const int idx = blockIdx.x * W + line;                    // row (row pass) or column (column pass)
+    const size_t gstride = COL ? (size_t)N : (size_t)1;
+    C *g = a.wf + (size_t)b * N * N + (COL ? (size_t)idx : (size_t)idx * N);
+
+    C v[16];
+#pragma unroll
+    for (int r = 0; r < 16; ++r) v[r] = g[(size_t)(j + r * TL) * gstride];
+
+    if constexpr (!COL) {
+        if (a.opd != nullptr) {
+            const T il = (T)a.inv_lambda[b];
+            const T *o = a.opd + (size_t)idx * N;
+#pragma unroll
+            for (int r = 0; r < 16; ++r) v[r] = cmul(v[r], phasor_turns(o[j + r * TL] * il));
+        }
+        if (a.amp != nullptr) {
+            const T *m = a.amp + (size_t)idx * N;
+#pragma unroll
+            for (int r = 0; r < 16; ++r) {
+                T s = m[j + r * TL];
+                v[r].x *= s; v[r].y *= s;
+            }
+        }
+    }
+    if (a.pre != nullptr) {
+        const C *p = a.pre + (size_t)b * N;
+#pragma unroll
+        for (int r = 0; r < 16; ++r) v[r] = cmul(v[r], ldg_c(p + j + r * TL));
+    }
+
+    if constexpr (MODE == MODE_INV) fft_line<T, N, +1, COL, W>(v, buf, line, j, a.tw);
+    else                            fft_line<T, N, -1, COL, W>(v, buf, line, j, a.tw);
+
+    if (a.mid != nullptr) {
+        const C *m = a.mid + (size_t)b * N;
+#pragma unroll
+        for (int r = 0; r < 16; ++r) v[r] = cmul(v[r], ldg_c(m + j + r * TL));
+    }
+
+    if constexpr (MODE == MODE_CONV) fft_line<T, N, +1, COL, W>(v, buf, line, j, a.tw);
+
+    if (a.scale != (T)1) {
+#pragma unroll
+        for (int r = 0; r < 16; ++r) { v[r].x *= a.scale; v[r].y *= a.scale; }
+    }
+#pragma unroll
+    for (int r = 0; r < 16; ++r) g[(size_t)(j + r * TL) * gstride] = v[r];
+}
+
+// ---- launch geometry -------------------------------------------------------------------------------
+// Lines per CTA.  Row pass: enough rows to make a CTA of >= 128 threads.  Column pass: W adjacent
+// columns so that every global access touches W*sizeof(complex) contiguous bytes per row
+// (>= 32 B sectors; 64 B where registers allow).
+template <typename T, int N, bool COL> struct PassGeom {
+    static constexpr int TL = N / 16;
+    static constexpr int ES = (int)sizeof(typename cplx_of<T>::type);
+    static constexpr int row_lines = TL >= 128 ? 1 : 128 / TL;
+    // column tile width: 64 B segments where the register file allows it (the tile lives in
+    // registers: 16 elements per thread, <= 512 threads for double, <= 1024 for float)
+    static constexpr int col_want = 64 / ES;
+    static constexpr int max_threads = sizeof(T) == 8 ? 512 : 1024;
+    static constexpr int col_max_by_threads = (max_threads / TL) < 1 ? 1 : (max_threads / TL);
+    static constexpr int col_lines = col_want < col_max_by_threads ? col_want : col_max_by_threads;
+    static constexpr int W = COL ? col_lines : row_lines;
+    static constexpr int threads = W * TL;
+    static constexpr size_t smem = (size_t)W * fr_padded_len(N) * ES;
+    // resident CTAs per SM the register budget is tuned for
+    static constexpr int regs_per_thread_goal = sizeof(T) == 8 ? 128 : 80;
+    static constexpr int minb_regs = 65536 / (threads * regs_per_thread_goal);
+    static constexpr int minb_smem = (int)((227 * 1024) / smem);
+    static constexpr int minb0 = minb_regs < minb_smem ? minb_regs : minb_smem;
+    static constexpr int MINB = minb0 < 1 ? 1 : (minb0 > 8 ? 8 : minb0);
+};
+
+template <typename T, int N, bool COL, int MODE>
+cudaError_t launch_pass(const PassArgs<T> &a, int batch, cudaStream_t stream)
+{
+    using G = PassGeom<T, N, COL>;
+    auto kern = pass_kernel<T, N, COL, G::W, MODE, G::MINB>;
+    static bool configured = false;     // per instantiation; attribute is per-device but we target one GPU per process
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::smem);
+        if (e != cudaSuccess) return e;
+        configured = true;
+    }
+    dim3 grid(N / G::W, batch, 1);
+    kern<<<grid, G::threads, G::smem, stream>>>(a);
+    return cudaGetLastError();
+}
+
+} // namespace fresnel

@@ -1,0 +1,298 @@
+"""GPU-vs-oracle parity (run with -m gpu on a B200).  Every call goes through the C ABI of
+libfresnel.so (paper_1806_06467_b200.binding); the expected values come from oracle/ on the same
+seeded inputs.  Bar (BASELINE.json:north_star): relative L2 per batch element, max over the batch,
+<= 1e-11 for complex128 and <= 2e-5 for complex64.  For c64 the inputs are rounded to float32
+first and the oracle runs in double on those rounded values.
+"""
+import math
+
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+TOL = {"c128": 1e-11, "c64": 2e-5}
+ALL_N = [64, 128, 256, 512, 1024, 2048]
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    return torch
+
+
+@pytest.fixture(scope="module")
+def B(torch_cuda):
+    from paper_1806_06467_b200 import binding
+    binding.lib()          # fails loudly if libfresnel.so is missing
+    return binding
+
+
+def rel_batch(got, want):
+    got = np.asarray(got).reshape(want.shape)
+    errs = [np.linalg.norm(got[b] - want[b]) / np.linalg.norm(want[b]) for b in range(want.shape[0])]
+    return float(max(errs))
+
+
+def field(N, seed, batch=1, dtype="c128"):
+    from paper_1806_06467_b200 import inputs
+    u = inputs.random_field(N, seed, batch)
+    if dtype == "c64":
+        u = u.astype(np.complex64).astype(np.complex128)
+    return u
+
+
+def to_dev(torch, u, dtype):
+    t = torch.from_numpy(np.ascontiguousarray(u))
+    if dtype == "c64":
+        t = t.to(torch.complex64)
+    return t.cuda().contiguous()
+
+
+def map_dev(torch, m, dtype):
+    if m is None:
+        return None
+    t = torch.from_numpy(np.ascontiguousarray(m))
+    return (t.to(torch.float32) if dtype == "c64" else t).cuda().contiguous()
+
+
+def map_host(m, dtype):
+    """what the GPU sees: for c64 the maps are float32"""
+    if m is None:
+        return None
+    return m.astype(np.float32).astype(np.float64) if dtype == "c64" else m
+
+
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("dtype", ["c128", "c64"])
+@pytest.mark.parametrize("N", ALL_N)
+@pytest.mark.parametrize("direction,centered", [(+1, False), (-1, False), (+1, True), (-1, True)])
+def test_fft2d(torch_cuda, B, oracle, N, dtype, direction, centered):
+    u = field(N, 100 + N, 2, dtype)
+    plan = B.Plan(N, 2, dtype)
+    d = to_dev(torch_cuda, u, dtype)
+    plan.fft2d(d, direction, centered)
+    want = np.stack([oracle.fft2d(u[b], direction, centered) for b in range(2)])
+    assert rel_batch(d.cpu().numpy(), want) <= TOL[dtype]
+
+
+@pytest.mark.parametrize("dtype", ["c128", "c64"])
+@pytest.mark.parametrize("N", ALL_N)
+def test_propagate_as(torch_cuda, B, oracle, N, dtype):
+    """config-4 style: random field, lambda 1e-6, z 0.5, dx 1e-5; two batch elements with different
+    wavelength and pitch so that per-batch tables are exercised."""
+    u = field(N, 4000 + int(math.log2(N)), 2, dtype)
+    dx, lam, z = np.array([1e-5, 1.3e-5]), np.array([1e-6, 0.7e-6]), 0.5
+    plan = B.Plan(N, 2, dtype)
+    d = to_dev(torch_cuda, u, dtype)
+    plan.propagate_as(d, dx, lam, z)
+    want = oracle.propagate_as_batch(u, dx, lam, z)
+    assert rel_batch(d.cpu().numpy(), want) <= TOL[dtype]
+    # negative z undoes it (g10)
+    plan.propagate_as(d, dx, lam, -z)
+    assert rel_batch(d.cpu().numpy(), u) <= 4 * TOL[dtype]
+
+
+@pytest.mark.parametrize("dtype", ["c128", "c64"])
+@pytest.mark.parametrize("N", [64, 256, 1024, 2048])
+@pytest.mark.parametrize("z", [0.7, -0.4])
+def test_propagate_direct(torch_cuda, B, oracle, N, dtype, z):
+    u = field(N, 200 + N, 2, dtype)
+    dx, lam = np.array([2e-5, 1.5e-5]), np.array([1e-6, 0.633e-6])
+    plan = B.Plan(N, 2, dtype)
+    d = to_dev(torch_cuda, u, dtype)
+    dx_out = plan.propagate_direct(d, dx, lam, z)
+    want = []
+    for b in range(2):
+        w, dxo = oracle.propagate_direct(u[b], dx[b], lam[b], z)
+        assert dx_out[b] == pytest.approx(dxo, rel=1e-15)
+        want.append(w)
+    assert rel_batch(d.cpu().numpy(), np.stack(want)) <= TOL[dtype]
+
+
+@pytest.mark.parametrize("dtype", ["c128", "c64"])
+@pytest.mark.parametrize("N", [64, 512, 2048])
+def test_apply_qpf_and_mask(torch_cuda, B, oracle, N, dtype):
+    from paper_1806_06467_b200 import inputs
+    u = field(N, 300 + N, 2, dtype)
+    dx, lam, f = np.array([2e-5, 1e-5]), np.array([550e-9, 600e-9]), 0.2     # corner phase ~ 1e3..2e4 rad
+    plan = B.Plan(N, 2, dtype)
+    d = to_dev(torch_cuda, u, dtype)
+    plan.apply_qpf(d, dx, lam, -f)
+    want = np.stack([oracle.apply_qpf(u[b], dx[b], lam[b], -f) for b in range(2)])
+    assert rel_batch(d.cpu().numpy(), want) <= TOL[dtype]
+
+    amp = inputs.circular_aperture(N, N / 3)
+    opd = inputs.psd_map(N, 2e-5, 3.0, 20e-9, 77)
+    for a, o in [(amp, opd), (None, opd), (amp, None)]:
+        d = to_dev(torch_cuda, u, dtype)
+        plan.apply_mask(d, map_dev(torch_cuda, a, dtype), map_dev(torch_cuda, o, dtype), lam)
+        want = np.stack([oracle.apply_mask(u[b], map_host(a, dtype), map_host(o, dtype), lam[b]) for b in range(2)])
+        assert rel_batch(d.cpu().numpy(), want) <= TOL[dtype]
+    # both NULL: no-op
+    d = to_dev(torch_cuda, u, dtype)
+    plan.apply_mask(d, None, None, lam)
+    assert rel_batch(d.cpu().numpy(), u) <= (1e-7 if dtype == "c64" else 0.0)
+
+
+@pytest.mark.parametrize("dtype", ["c128", "c64"])
+@pytest.mark.parametrize("N", [128, 1024, 2048])
+def test_surface_as_fused_vs_oracle_and_primitives(torch_cuda, B, oracle, N, dtype):
+    from paper_1806_06467_b200 import inputs
+    u = field(N, 500 + N, 2, dtype)
+    dx, lam, f, z = np.array([2e-5, 2e-5]), np.array([550e-9, 640e-9]), 0.8, 0.35
+    amp = inputs.circular_aperture(N, N / 4)
+    opd = inputs.psd_map(N, 2e-5, 3.0, 10e-9, 78)
+    plan = B.Plan(N, 2, dtype)
+    da, do = map_dev(torch_cuda, amp, dtype), map_dev(torch_cuda, opd, dtype)
+    d = to_dev(torch_cuda, u, dtype)
+    plan.surface_as(d, dx, lam, f, da, do, z)
+    want = oracle.surface_as_batch(u, dx, lam, f, map_host(amp, dtype), map_host(opd, dtype), z)
+    assert rel_batch(d.cpu().numpy(), want) <= TOL[dtype]
+    # fused == primitives chained, to rounding
+    e = to_dev(torch_cuda, u, dtype)
+    plan.apply_qpf(e, dx, lam, -f)
+    plan.apply_mask(e, da, do, lam)
+    plan.propagate_as(e, dx, lam, z)
+    assert rel_batch(e.cpu().numpy(), d.cpu().numpy().reshape(2, N, N)) <= TOL[dtype]
+    # z == 0: optic only
+    g = to_dev(torch_cuda, u, dtype)
+    plan.surface_as(g, dx, lam, f, da, do, 0.0)
+    want0 = np.stack([oracle.apply_mask(oracle.apply_qpf(u[b], dx[b], lam[b], -f), map_host(amp, dtype),
+                                        map_host(opd, dtype), lam[b]) for b in range(2)])
+    assert rel_batch(g.cpu().numpy(), want0) <= TOL[dtype]
+
+
+def test_config1(torch_cuda, B, oracle):
+    from paper_1806_06467_b200 import inputs
+    wl = inputs.config1()
+    plan = B.Plan(wl.N, 1, "c128")
+    d = to_dev(torch_cuda, wl.field, "c128")
+    plan.propagate_as(d, wl.dx, wl.lam, wl.surfaces[0].z)
+    want = oracle.propagate_as_batch(wl.field, wl.dx, wl.lam, wl.surfaces[0].z)
+    assert rel_batch(d.cpu().numpy(), want) <= 1e-11
+
+
+def test_config2_both_variants(torch_cuda, B, oracle):
+    """Gaussian-beam chain: GPU vs oracle after every stage, AS and direct variants."""
+    from paper_1806_06467_b200 import inputs
+    wl = inputs.config2()
+    lam = wl.lam
+    plan = B.Plan(wl.N, 1, "c128")
+    d = to_dev(torch_cuda, wl.field, "c128")
+    o = wl.field[0]
+    for s in wl.surfaces:
+        plan.surface_as(d, wl.dx, lam, s.f, None, None, s.z)
+        o = oracle.surface_as(o, wl.dx[0], lam[0], s.f, None, None, s.z)
+        assert rel_batch(d.cpu().numpy(), o[None]) <= 1e-11
+    d = to_dev(torch_cuda, wl.field, "c128")
+    o, dx_o, dx_g = wl.field[0], float(wl.dx[0]), wl.dx.copy()
+    for s in wl.surfaces:
+        plan.apply_qpf(d, dx_g, lam, -s.f)
+        dx_g = plan.propagate_direct(d, dx_g, lam, s.z)
+        o = oracle.apply_qpf(o, dx_o, lam[0], -s.f)
+        o, dx_o = oracle.propagate_direct(o, dx_o, lam[0], s.z)
+        assert dx_g[0] == pytest.approx(dx_o, rel=1e-15)
+        assert rel_batch(d.cpu().numpy(), o[None]) <= 1e-11
+
+
+def test_config3_reduced_chain(torch_cuda, B, oracle):
+    """Shaped-pupil-coronagraph analog at N=512 (full recipe, scaled masks), all 20 surfaces."""
+    from paper_1806_06467_b200 import inputs
+    wl = inputs.config3(N=512)
+    plan = B.Plan(wl.N, 1, "c128")
+    d = to_dev(torch_cuda, wl.field, "c128")
+    o = wl.field[0]
+    for i, s in enumerate(wl.surfaces):
+        plan.surface_as(d, wl.dx, wl.lam, s.f, map_dev(torch_cuda, s.amp, "c128"), map_dev(torch_cuda, s.opd, "c128"), s.z)
+        o = oracle.surface_as(o, wl.dx[0], wl.lam[0], s.f, s.amp, s.opd, s.z)
+        if i in (0, 6, 12, 19):
+            assert rel_batch(d.cpu().numpy(), o[None]) <= 1e-11, f"surface {i}"
+
+
+def test_config5_reduced_batch(torch_cuda, B, oracle):
+    """Polychromatic batch at N=512, 4 wavelengths, 10 planes, c64."""
+    from paper_1806_06467_b200 import inputs
+    wl = inputs.config5(N=512, batch=4)
+    plan = B.Plan(wl.N, wl.batch, "c64")
+    d = to_dev(torch_cuda, wl.field, "c64")
+    o = wl.field.copy()
+    for s in wl.surfaces:
+        plan.surface_as(d, wl.dx, wl.lam, s.f, map_dev(torch_cuda, s.amp, "c64"), map_dev(torch_cuda, s.opd, "c64"), s.z)
+        o = oracle.surface_as_batch(o, wl.dx, wl.lam, s.f, map_host(s.amp, "c64"), map_host(s.opd, "c64"), s.z)
+    assert rel_batch(d.cpu().numpy(), o) <= 2e-5
+
+
+@pytest.mark.parametrize("dtype,N", [("c128", 4096), ("c64", 4096), ("c64", 8192), ("c128", 8192)])
+def test_large_grids_sampled(torch_cuda, B, oracle, dtype, N):
+    """Full bench sizes: the oracle's radix-2 FFT still finishes in seconds at 4096/8192, so compare
+    the whole field for one AS step of config 4."""
+    from paper_1806_06467_b200 import inputs
+    wl = inputs.config4(N, dtype)
+    plan = B.Plan(N, 1, dtype)
+    d = to_dev(torch_cuda, wl.field, dtype)
+    plan.propagate_as(d, wl.dx, wl.lam, wl.surfaces[0].z)
+    want = oracle.propagate_as_batch(wl.field, wl.dx, wl.lam, wl.surfaces[0].z)
+    assert rel_batch(d.cpu().numpy(), want) <= TOL[dtype]
+
+
+def test_error_codes(torch_cuda, B):
+    import ctypes
+    L = B.lib()
+    h = ctypes.c_void_p()
+    assert L.fresnel_plan_create(ctypes.byref(h), 2800, 1, 1) == 2          # UNSUPPORTED (g12)
+    assert L.fresnel_plan_create(ctypes.byref(h), 32, 1, 1) == 2
+    assert L.fresnel_plan_create(ctypes.byref(h), 256, 0, 1) == 1           # INVALID_ARG
+    assert L.fresnel_plan_create(None, 256, 1, 1) == 1
+    plan = B.Plan(256, 1, "c128")
+    d = torch_cuda.zeros(256, 256, dtype=torch_cuda.complex128, device="cuda")
+    with pytest.raises(B.FresnelError):
+        plan.apply_qpf(d, [1e-5], [1e-6], 0.0)
+    with pytest.raises(B.FresnelError):
+        plan.propagate_direct(d, [1e-5], [1e-6], 0.0)
+    with pytest.raises(B.FresnelError):
+        plan.propagate_as(d, [1e-5], [-1e-6], 0.1)
+    with pytest.raises(B.FresnelError):
+        plan.propagate_as(d, [0.0], [1e-6], 0.1)
+    with pytest.raises(B.FresnelError):
+        plan.propagate_as(d, [1e-5], [1e-6], float("nan"))
+    with pytest.raises(B.FresnelError):
+        plan.fft2d(d, 0, False)
+    with pytest.raises(B.FresnelError):
+        plan.surface_as(d, [1e-5], [1e-6], 0.0, None, None, 0.1)
+    # z = 0 AS is the identity and launches nothing
+    n0 = plan.launch_count()
+    plan.propagate_as(d, [1e-5], [1e-6], 0.0)
+    assert plan.launch_count() == n0
+    assert L.fresnel_plan_destroy(None) == 0
+
+
+def test_cuda_graph_capture_of_a_chain(torch_cuda, B, oracle):
+    """Hot calls enqueue only (no allocation, no sync): a chain can be captured and replayed."""
+    torch = torch_cuda
+    from paper_1806_06467_b200 import inputs
+    wl = inputs.config2()
+    s = torch.cuda.Stream()
+    plan = B.Plan(wl.N, 1, "c128", stream=s)
+    d = to_dev(torch, wl.field, "c128")
+    src = d.clone()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(s):
+        for surf in wl.surfaces:                       # warm-up outside capture
+            plan.surface_as(d, wl.dx, wl.lam, surf.f, None, None, surf.z)
+        s.synchronize()
+        d.copy_(src)
+        s.synchronize()
+        with torch.cuda.graph(g, stream=s):
+            for surf in wl.surfaces:
+                plan.surface_as(d, wl.dx, wl.lam, surf.f, None, None, surf.z)
+    d.copy_(src)
+    torch.cuda.synchronize()
+    g.replay()
+    torch.cuda.synchronize()
+    o = wl.field[0]
+    for surf in wl.surfaces:
+        o = oracle.surface_as(o, wl.dx[0], wl.lam[0], surf.f, None, None, surf.z)
+    assert rel_batch(d.cpu().numpy(), o[None]) <= 1e-11

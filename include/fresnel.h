@@ -75,6 +75,13 @@ fresnel_status fresnel_plan_destroy(fresnel_plan *p);
 /* Number of kernels this plan has launched so far (bench.py reports it as gpu_launches). */
 fresnel_status fresnel_plan_launch_count(const fresnel_plan *p, unsigned long long *count);
 
+/* Profiling hook (used by bench.py to time the row and the column kernel inside the real timed
+ * region): the NEXT two-pass call on this plan (fresnel_fft2d, fresnel_propagate_as,
+ * fresnel_propagate_direct, fresnel_surface_as with z != 0) records events[0] before its row
+ * pass, events[1] between the passes and events[2] after its column pass, on the plan's stream.
+ * events: HOST array of 3 cudaEvent_t handles owned by the caller (passed as void*); NULL disarms. */
+fresnel_status fresnel_plan_record_pass_events(fresnel_plan *p, void *const events[3]);
+
 /* ---- the operations of the hot path ----------------------------------------------------------- */
 
 /* Quadratic phase factor, Eq. 2 read as (g1)

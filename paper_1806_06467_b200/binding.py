@@ -17,7 +17,7 @@ from typing import Optional, Sequence
 import numpy as np
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(HERE, "libfresnel.so")
+LIB_PATH = os.environ.get("FRESNEL_LIB", os.path.join(HERE, "libfresnel.so"))   # override: tuning builds only
 
 FRESNEL_OK = 0
 FORWARD = +1
@@ -27,7 +27,7 @@ C64, C128 = 0, 1
 # every symbol include/fresnel.h declares (tests/test_abi.py checks the header against this list)
 SYMBOLS = (
     "fresnel_plan_create", "fresnel_plan_set_stream", "fresnel_plan_synchronize", "fresnel_plan_destroy",
-    "fresnel_plan_launch_count", "fresnel_apply_qpf", "fresnel_apply_mask", "fresnel_fft2d",
+    "fresnel_plan_launch_count", "fresnel_plan_record_pass_events", "fresnel_apply_qpf", "fresnel_apply_mask", "fresnel_fft2d",
     "fresnel_propagate_as", "fresnel_propagate_direct", "fresnel_surface_as", "fresnel_memcpy_h2d",
     "fresnel_memcpy_d2h", "fresnel_status_string", "fresnel_version",
 )
@@ -57,6 +57,7 @@ def lib() -> ctypes.CDLL:
     L.fresnel_plan_synchronize.argtypes = [vp]
     L.fresnel_plan_destroy.argtypes = [vp]
     L.fresnel_plan_launch_count.argtypes = [vp, ctypes.POINTER(ctypes.c_ulonglong)]
+    L.fresnel_plan_record_pass_events.argtypes = [vp, ctypes.POINTER(vp)]
     L.fresnel_apply_qpf.argtypes = [vp, vp, dp, dp, cd]
     L.fresnel_apply_mask.argtypes = [vp, vp, vp, vp, dp]
     L.fresnel_fft2d.argtypes = [vp, vp, ci, ci]
@@ -117,6 +118,17 @@ class Plan:
         c = ctypes.c_ulonglong(0)
         self._chk(lib().fresnel_plan_launch_count(self._h, ctypes.byref(c)), "fresnel_plan_launch_count")
         return int(c.value)
+
+    def record_pass_events(self, events) -> None:
+        """Arm the profiling hook with 3 torch.cuda.Event(enable_timing=True) objects (or None)."""
+        if events is None:
+            self._chk(lib().fresnel_plan_record_pass_events(self._h, None), "fresnel_plan_record_pass_events")
+            return
+        for e in events:
+            if not e.cuda_event:          # torch creates the handle lazily on first record()
+                e.record(self._stream)
+        arr = (ctypes.c_void_p * 3)(*[ctypes.c_void_p(e.cuda_event) for e in events])
+        self._chk(lib().fresnel_plan_record_pass_events(self._h, arr), "fresnel_plan_record_pass_events")
 
     def close(self) -> None:
         if getattr(self, "_h", None) is not None and self._h.value:

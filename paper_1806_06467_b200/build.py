@@ -16,7 +16,9 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
-LIB = os.path.join(HERE, "libfresnel.so")
+# FRESNEL_LIB_NAME / FRESNEL_DEFINES: tuning builds only (e.g. FRESNEL_DEFINES="-DFR_COLW_F64=4")
+LIB = os.path.join(HERE, os.environ.get("FRESNEL_LIB_NAME", "libfresnel.so"))
+EXTRA_DEFINES = os.environ.get("FRESNEL_DEFINES", "").split()
 SIZES = (64, 128, 256, 512, 1024, 2048, 4096, 8192)
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr"]
@@ -37,13 +39,13 @@ def _sources_digest() -> str:
                 with open(os.path.join(root, name), "rb") as fh:
                     h.update(name.encode())
                     h.update(fh.read())
-    h.update(" ".join(NVCC_FLAGS).encode())
+    h.update(" ".join(NVCC_FLAGS + EXTRA_DEFINES).encode())
     return h.hexdigest()
 
 
 def _compile(args):
     src, obj, extra = args
-    cmd = [_nvcc(), *NVCC_FLAGS, *extra, "-c", src, "-o", obj]
+    cmd = [_nvcc(), *NVCC_FLAGS, *EXTRA_DEFINES, *extra, "-c", src, "-o", obj]
     r = subprocess.run(cmd, capture_output=True, text=True)
     if r.returncode != 0:
         raise RuntimeError(f"nvcc failed: {' '.join(cmd)}\n{r.stdout}\n{r.stderr}")
@@ -52,7 +54,7 @@ def _compile(args):
 
 def build(force: bool = False, verbose: bool = False) -> str:
     os.makedirs(OBJ, exist_ok=True)
-    stamp = os.path.join(OBJ, "digest.txt")
+    stamp = os.path.join(OBJ, os.path.basename(LIB) + ".digest.txt")
     digest = _sources_digest()
     if not force and os.path.exists(LIB) and os.path.exists(stamp) and open(stamp).read() == digest:
         return LIB

@@ -33,6 +33,8 @@ template <typename C> FR_DEV C cmulc(C a, C b) { C r; r.x = a.x * b.x + a.y * b.
 
 // DIR = -1: forward kernel exp(-2 pi i ...); DIR = +1: inverse kernel.  Tables hold FORWARD twiddles.
 template <int DIR, typename C> FR_DEV C twmul(C a, C w) { return DIR < 0 ? cmul(a, w) : cmulc(a, w); }
+// w * w
+template <typename C> FR_DEV C csq(C w) { C r; r.x = w.x * w.x - w.y * w.y; r.y = (w.x + w.x) * w.y; return r; }
 
 // multiply by -i (DIR<0) or +i (DIR>0):  the radix-4 quarter turn
 template <int DIR, typename C> FR_DEV C rot90(C a)
@@ -150,11 +152,14 @@ __host__ __device__ constexpr int fr_ns(int N, int stage)      // product of the
     return ns;
 }
 // offset (in complex elements) of stage `stage`'s twiddle table inside the per-N table; stage >= 1.
-// Layout of a stage table: [t-1][k], t = 1..R-1, k = 0..Ns-1  (k contiguous => coalesced reads).
+// A stage table holds only the BASE twiddles w_k = W_{Ns*R}^k, k = 0..Ns-1 (exactly rounded, built
+// in long double on the host).  The powers w_k^t, t = 2..R-1, are generated in registers by at most
+// five chained multiplications: one 16-byte load costs the load/store pipe as much as eight FP64
+// instructions cost the FP64 pipe, a complex multiply is four.
 __host__ __device__ constexpr int fr_tw_offset(int N, int stage)
 {
     int off = 0;
-    for (int s = 1; s < stage; ++s) off += (fr_radix(N, s) - 1) * fr_ns(N, s);
+    for (int s = 1; s < stage; ++s) off += fr_ns(N, s);
     return off;
 }
 __host__ __device__ constexpr int fr_tw_total(int N) { return fr_tw_offset(N, fr_num_stages(N)); }
@@ -187,14 +192,31 @@ FR_DEV void fft_stage(typename cplx_of<T>::type (&v)[16], typename cplx_of<T>::t
     constexpr bool LAST = (STAGE == fr_num_stages(N) - 1);
     static_assert(LAST || R == 16, "only the last stage may have a radix below 16");
 
-    // ---- twiddles (none in the first stage: Ns = 1) ----
+    // ---- twiddles (none in the first stage: Ns = 1): v[b + q*B] *= w^q, w = W_{Ns*R}^k ----
     if constexpr (STAGE > 0) {
         const C *t = tw + fr_tw_offset(N, STAGE);
 #pragma unroll
         for (int b = 0; b < B; ++b) {
             const int k = (j + b * TL) & (NS - 1);
+            const C p1 = ldg_c(t + k);
+            v[b + B] = twmul<DIR>(v[b + B], p1);
+            if constexpr (R >= 4) {
+                const C p2 = csq(p1), p3 = cmul(p2, p1);
+                v[b + 2 * B] = twmul<DIR>(v[b + 2 * B], p2);
+                v[b + 3 * B] = twmul<DIR>(v[b + 3 * B], p3);
+                if constexpr (R >= 8) {
+                    const C p4 = csq(p2);
+                    C g = p4;                                        // w^(4m)
 #pragma unroll
-            for (int q = 1; q < R; ++q) v[b + q * B] = twmul<DIR>(v[b + q * B], ldg_c(t + (q - 1) * NS + k));
+                    for (int m = 1; m < R / 4; ++m) {                // block m: w^(4m) .. w^(4m+3)
+                        v[b + (4 * m) * B] = twmul<DIR>(v[b + (4 * m) * B], g);
+                        v[b + (4 * m + 1) * B] = twmul<DIR>(v[b + (4 * m + 1) * B], cmul(g, p1));
+                        v[b + (4 * m + 2) * B] = twmul<DIR>(v[b + (4 * m + 2) * B], cmul(g, p2));
+                        v[b + (4 * m + 3) * B] = twmul<DIR>(v[b + (4 * m + 3) * B], cmul(g, p3));
+                        if (m + 1 < R / 4) g = (m == 1) ? csq(g) : cmul(g, p4);   // w^8 = (w^4)^2, w^12 = w^8 * w^4
+                    }
+                }
+            }
         }
     }
     // ---- butterflies ----

@@ -48,6 +48,8 @@ struct fresnel_plan {
     TableSlot slots[kSlots];
     uint64_t clock = 0, call_id = 0;
     unsigned long long launches = 0;
+    cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};   // profiling hook, see fresnel_plan_record_pass_events
+    bool ev_armed = false;
     size_t esize() const { return dtype == FRESNEL_C128 ? sizeof(double2) : sizeof(float2); }
 };
 
@@ -63,15 +65,14 @@ template <typename C> void fill_twiddles_for(int N, std::vector<C> &out)
     for (int s = 1; s < S; ++s) {
         const int R = fr_radix(N, s), NS = fr_ns(N, s);
         C *t = out.data() + fr_tw_offset(N, s);
-        for (int q = 1; q < R; ++q)
-            for (int k = 0; k < NS; ++k) {
-                // forward twiddle W_{NS*R}^{q*k} = exp(-2 pi i q k / (NS*R)); q*k < NS*R always
-                long double ang = -2.0L * PI_L * (long double)((long)q * k) / (long double)((long)NS * R);
-                C w;
-                w.x = (decltype(w.x))cosl(ang);
-                w.y = (decltype(w.y))sinl(ang);
-                t[(size_t)(q - 1) * NS + k] = w;
-            }
+        for (int k = 0; k < NS; ++k) {
+            // base forward twiddle W_{NS*R}^k = exp(-2 pi i k / (NS*R)); its powers are formed on the device
+            long double ang = -2.0L * PI_L * (long double)k / (long double)((long)NS * R);
+            C w;
+            w.x = (decltype(w.x))cosl(ang);
+            w.y = (decltype(w.y))sinl(ang);
+            t[k] = w;
+        }
     }
 }
 
@@ -227,6 +228,22 @@ fresnel_status run_pass(fresnel_plan *p, bool col, int mode, void *wf, const voi
     return FRESNEL_OK;
 }
 
+// The two HBM round trips of a propagation / transform: row pass then column pass.
+fresnel_status run_two_passes(fresnel_plan *p, int mode, void *wf, const void *pre, const void *mid,
+                              const void *amp, const void *opd, double scale)
+{
+    const bool ev = p->ev_armed;
+    p->ev_armed = false;
+    if (ev && cudaEventRecord(p->ev[0], p->stream) != cudaSuccess) return FRESNEL_ERR_CUDA;
+    fresnel_status st = run_pass(p, false, mode, wf, pre, mid, amp, opd, scale);
+    if (st != FRESNEL_OK) return st;
+    if (ev && cudaEventRecord(p->ev[1], p->stream) != cudaSuccess) return FRESNEL_ERR_CUDA;
+    st = run_pass(p, true, mode, wf, pre, mid, nullptr, nullptr, scale);
+    if (st != FRESNEL_OK) return st;
+    if (ev && cudaEventRecord(p->ev[2], p->stream) != cudaSuccess) return FRESNEL_ERR_CUDA;
+    return FRESNEL_OK;
+}
+
 fresnel_status run_pointwise(fresnel_plan *p, void *wf, const void *tab, const void *amp, const void *opd)
 {
     cudaError_t e;
@@ -323,6 +340,18 @@ fresnel_status fresnel_plan_launch_count(const fresnel_plan *p, unsigned long lo
     return FRESNEL_OK;
 }
 
+fresnel_status fresnel_plan_record_pass_events(fresnel_plan *p, void *const events[3])
+{
+    if (!p) return FRESNEL_ERR_INVALID_ARG;
+    if (!events) { p->ev_armed = false; return FRESNEL_OK; }
+    for (int i = 0; i < 3; ++i) {
+        if (!events[i]) return FRESNEL_ERR_INVALID_ARG;
+        p->ev[i] = (cudaEvent_t)events[i];
+    }
+    p->ev_armed = true;
+    return FRESNEL_OK;
+}
+
 fresnel_status fresnel_memcpy_h2d(fresnel_plan *p, void *dst_device, const void *src_host, size_t bytes)
 {
     if (!p || !dst_device || !src_host) return FRESNEL_ERR_INVALID_ARG;
@@ -371,9 +400,7 @@ fresnel_status fresnel_fft2d(fresnel_plan *p, void *wf, int direction, int cente
     const int mode = direction == FRESNEL_FORWARD ? MODE_FWD : MODE_INV;
     const double per_pass = direction == FRESNEL_FORWARD ? 1.0 : 1.0 / (double)p->N;
     if (!centered) {
-        fresnel_status st = run_pass(p, false, mode, wf, nullptr, nullptr, nullptr, nullptr, per_pass);
-        if (st != FRESNEL_OK) return st;
-        return run_pass(p, true, mode, wf, nullptr, nullptr, nullptr, nullptr, per_pass);
+        return run_two_passes(p, mode, wf, nullptr, nullptr, nullptr, nullptr, per_pass);
     }
     // centred transform = s * fft2(s * u), s = (-1)^(j+k): sign tables on load and after the transform
     const bool force = capturing(p);
@@ -382,9 +409,7 @@ fresnel_status fresnel_fft2d(fresnel_plan *p, void *wf, int direction, int cente
     if (r[0].slot == r[1].slot) r[1].build = false;
     fresnel_status st = flush_builds(p, r, 2, nullptr);
     if (st != FRESNEL_OK) return st;
-    st = run_pass(p, false, mode, wf, p->slots[r[0].slot].dev, p->slots[r[1].slot].dev, nullptr, nullptr, 1.0);
-    if (st != FRESNEL_OK) return st;
-    return run_pass(p, true, mode, wf, p->slots[r[0].slot].dev, p->slots[r[1].slot].dev, nullptr, nullptr, 1.0);
+    return run_two_passes(p, mode, wf, p->slots[r[0].slot].dev, p->slots[r[1].slot].dev, nullptr, nullptr, 1.0);
 }
 
 // ---- fused surface: lens + optic phasor + angular-spectrum propagation ----------------------------
@@ -419,11 +444,9 @@ fresnel_status fresnel_surface_as(fresnel_plan *p, void *wf, const double *pixel
     const void *tl = lens ? p->slots[r[i_lens].slot].dev : nullptr;
     if (!prop) return run_pointwise(p, wf, tl, amp, opd);          // optic only
     const void *th = p->slots[r[i_h].slot].dev;
-    // row pass: optic phasor and x-chirp of the lens on load, FFT, x H1, inverse FFT
-    st = run_pass(p, false, MODE_CONV, wf, tl, th, amp, opd, 1.0);
-    if (st != FRESNEL_OK) return st;
+    // row pass: optic phasor and x-chirp of the lens on load, FFT, x H1, inverse FFT;
     // column pass: y-chirp of the lens on load, FFT, x H1, inverse FFT
-    return run_pass(p, true, MODE_CONV, wf, tl, th, nullptr, nullptr, 1.0);
+    return run_two_passes(p, MODE_CONV, wf, tl, th, amp, opd, 1.0);
 }
 
 fresnel_status fresnel_propagate_as(fresnel_plan *p, void *wf, const double *pixel, const double *lambda, double z)
@@ -454,9 +477,7 @@ fresnel_status fresnel_propagate_direct(fresnel_plan *p, void *wf, double *pixel
     fresnel_status st = flush_builds(p, r, 2, nullptr);
     if (st != FRESNEL_OK) return st;
     const int mode = z > 0 ? MODE_FWD : MODE_INV;
-    st = run_pass(p, false, mode, wf, p->slots[r[0].slot].dev, p->slots[r[1].slot].dev, nullptr, nullptr, 1.0);
-    if (st != FRESNEL_OK) return st;
-    st = run_pass(p, true, mode, wf, p->slots[r[0].slot].dev, p->slots[r[1].slot].dev, nullptr, nullptr, 1.0);
+    st = run_two_passes(p, mode, wf, p->slots[r[0].slot].dev, p->slots[r[1].slot].dev, nullptr, nullptr, 1.0);
     if (st != FRESNEL_OK) return st;
     for (int b = 0; b < p->batch; ++b) pixel_inout[b] = dx_out[b];
     return FRESNEL_OK;

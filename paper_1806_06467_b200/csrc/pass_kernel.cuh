@@ -106,23 +106,52 @@ __global__ void __launch_bounds__(W *(N / 16), MINB) pass_kernel(PassArgs<T> a)
 
 // ---- launch geometry -------------------------------------------------------------------------------
 // Lines per CTA.  Row pass: enough rows to make a CTA of >= 128 threads.  Column pass: W adjacent
-// columns so that every global access touches W*sizeof(complex) contiguous bytes per row
-// (>= 32 B sectors; 64 B where registers allow).
+// columns, so that a row of the tile is W*sizeof(complex) contiguous bytes (>= one 32 B sector),
+// chosen so that at least two CTAs fit an SM wherever the register file allows (the tile lives in
+// registers, 16 elements per thread; co-resident CTAs are what overlaps one tile's loads with
+// another tile's butterflies).  Override per build with -DFR_COLW_F64=<W> / -DFR_COLW_F32=<W>.
+__host__ __device__ constexpr int fr_col_lines(int N, int elem_bytes)
+{
+    const int TL = N / 16;
+    if (elem_bytes == 16) {
+#ifdef FR_COLW_F64
+        if (FR_COLW_F64 * TL <= 512) return FR_COLW_F64;
+#endif
+        return N <= 1024 ? 4 : (N <= 4096 ? 2 : 1);
+    }
+#ifdef FR_COLW_F32
+    if (FR_COLW_F32 * TL <= 1024) return FR_COLW_F32;
+#endif
+    return N <= 1024 ? 8 : (N <= 4096 ? 4 : 2);
+}
+__host__ __device__ constexpr int fr_row_lines(int N, int elem_bytes)
+{
+    const int TL = N / 16;
+#ifdef FR_ROWL_F64
+    if (elem_bytes == 16 && FR_ROWL_F64 * TL <= 512 && FR_ROWL_F64 * TL >= 128) return FR_ROWL_F64;
+#endif
+#ifdef FR_ROWL_F32
+    if (elem_bytes == 8 && FR_ROWL_F32 * TL <= 1024 && FR_ROWL_F32 * TL >= 128) return FR_ROWL_F32;
+#endif
+    return TL >= 128 ? 1 : 128 / TL;
+}
+
 template <typename T, int N, bool COL> struct PassGeom {
     static constexpr int TL = N / 16;
     static constexpr int ES = (int)sizeof(typename cplx_of<T>::type);
-    static constexpr int row_lines = TL >= 128 ? 1 : 128 / TL;
-    // column tile width: 64 B segments where the register file allows it (the tile lives in
-    // registers: 16 elements per thread, <= 512 threads for double, <= 1024 for float)
-    static constexpr int col_want = 64 / ES;
-    static constexpr int max_threads = sizeof(T) == 8 ? 512 : 1024;
-    static constexpr int col_max_by_threads = (max_threads / TL) < 1 ? 1 : (max_threads / TL);
-    static constexpr int col_lines = col_want < col_max_by_threads ? col_want : col_max_by_threads;
-    static constexpr int W = COL ? col_lines : row_lines;
+    static constexpr int row_lines = fr_row_lines(N, ES);
+    static constexpr int W = COL ? fr_col_lines(N, ES) : row_lines;
     static constexpr int threads = W * TL;
+    static_assert(threads <= 1024, "CTA too large");
     static constexpr size_t smem = (size_t)W * fr_padded_len(N) * ES;
     // resident CTAs per SM the register budget is tuned for
-    static constexpr int regs_per_thread_goal = sizeof(T) == 8 ? 128 : 80;
+#ifndef FR_REGS_F64
+#define FR_REGS_F64 128
+#endif
+#ifndef FR_REGS_F32
+#define FR_REGS_F32 64
+#endif
+    static constexpr int regs_per_thread_goal = sizeof(T) == 8 ? FR_REGS_F64 : FR_REGS_F32;
     static constexpr int minb_regs = 65536 / (threads * regs_per_thread_goal);
     static constexpr int minb_smem = (int)((227 * 1024) / smem);
     static constexpr int minb0 = minb_regs < minb_smem ? minb_regs : minb_smem;

@@ -1,0 +1,209 @@
+// col_tma.cuh -- the COLUMN pass with TMA tile movement (sm_100a).
+//
+// A column tile is [N rows] x [W adjacent columns]: W*sizeof(complex) contiguous bytes per row at a
+// pitch of N*sizeof(complex).  Gathered with per-thread loads this costs the load/store pipe one
+// wavefront per 128-byte line touched (8..32 per warp instruction instead of 4), which made the
+// column pass the slowest kernel.  Here one elected thread asks the TMA unit for the whole tile
+// (cp.async.bulk.tensor, boxes of 256 rows x W columns, hardware-swizzled so that a column can be
+// read back without bank conflicts); the tile lands in the shared memory that afterwards serves as
+// the exchange buffers, and goes back to HBM the same way.  The W columns of a tile are independent
+// transforms: each is owned by its own group of N/16 threads that synchronises on a private
+// named barrier, so the groups of a CTA drift apart and overlap one another's FP64 and
+// shared-memory phases.  Only the tile load and the tile store are CTA-wide events.
+#pragma once
+#include <cuda.h>
+#include <cstdint>
+#include "pass_kernel.cuh"
+
+namespace fresnel {
+
+FR_DEV uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+FR_DEV void mbar_init(uint64_t *bar, int count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+FR_DEV void mbar_expect_tx(uint64_t *bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+FR_DEV void mbar_wait(uint64_t *bar, uint32_t parity)
+{
+    uint32_t done;
+    do {
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                     : "=r"(done) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+    } while (!done);
+}
+FR_DEV void tma_load_3d(void *dst, const CUtensorMap *map, uint64_t *bar, int x, int y, int z)
+{
+    asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
+                 ::"r"(smem_u32(dst)), "l"(map), "r"(smem_u32(bar)), "r"(x), "r"(y), "r"(z) : "memory");
+}
+FR_DEV void tma_store_3d(const CUtensorMap *map, const void *src, int x, int y, int z)
+{
+    asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.bulk_group [%0, {%2, %3, %4}], [%1];"
+                 ::"l"(map), "r"(smem_u32(src)), "r"(x), "r"(y), "r"(z) : "memory");
+}
+FR_DEV void tma_store_commit_and_wait()
+{
+    asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+    asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");   // shared memory may be released
+}
+// L2 prefetch of a tile box (no shared-memory destination): the tile a later CTA will ask for
+FR_DEV void tma_prefetch_3d(const CUtensorMap *map, int x, int y, int z)
+{
+    asm volatile("cp.async.bulk.prefetch.tensor.3d.L2.global [%0, {%1, %2, %3}];" ::"l"(map), "r"(x), "r"(y), "r"(z) : "memory");
+}
+FR_DEV void fence_async_proxy() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
+// byte offset of element (row, col) of a [rows][W] tile written by TMA with the swizzle mode that
+// matches the row length (32 / 64 / 128 bytes): XOR of the 16-byte-chunk bits with address bits 7..9
+template <int ROW_BYTES> FR_DEV uint32_t tile_swizzle(uint32_t off)
+{
+    if constexpr (ROW_BYTES == 32) return off ^ ((off >> 3) & 0x10);
+    else if constexpr (ROW_BYTES == 64) return off ^ ((off >> 3) & 0x30);
+    else if constexpr (ROW_BYTES == 128) return off ^ ((off >> 3) & 0x70);
+    else return off;     // 16-byte rows: no swizzle
+}
+
+constexpr int kTmaBoxRows = 256;
+
+template <typename T, int N, int W, int MODE, int MINB>
+__global__ void __launch_bounds__(W *(N / 16), MINB)
+col_tma_kernel(PassArgs<T> a, const __grid_constant__ CUtensorMap tmap)
+{
+    using C = typename cplx_of<T>::type;
+    constexpr int TL = N / 16;                       // threads per column
+    constexpr int ES = (int)sizeof(C);
+    constexpr int ROW_BYTES = W * ES;
+    constexpr int GT = (W == 1) ? 0 : TL;            // group barrier size (W == 1: the CTA is the group)
+    extern __shared__ __align__(1024) unsigned char fr_smem[];
+    __shared__ __align__(8) uint64_t full_bar;
+    // 1024-byte alignment (the TMA swizzle pattern is a function of the shared-memory address)
+    unsigned char *tile = fr_smem + ((1024u - (smem_u32(fr_smem) & 1023u)) & 1023u);   // landing zone, later the exchange buffers
+    C *buf = reinterpret_cast<C *>(tile);
+
+    const int tid = threadIdx.x;
+    const int g = tid / TL;                          // column of the tile == thread group
+    const int j = tid % TL;
+    const int b = blockIdx.y;
+    const int col0 = blockIdx.x * W;
+
+    if (tid == 0) mbar_init(&full_bar, 1);
+    __syncthreads();
+    if (tid == 0) {
+        mbar_expect_tx(&full_bar, (uint32_t)(N * ROW_BYTES));
+#pragma unroll 1
+        for (int r0 = 0; r0 < N; r0 += kTmaBoxRows)
+            tma_load_3d(tile + (size_t)r0 * ROW_BYTES, &tmap, &full_bar, col0 * 2, r0, b);
+    }
+    // Ask L2 for the tile that the CTA taking over one of the currently resident slots will need
+    // (CTAs are dispatched in blockIdx order): HBM then streams while this tile is being computed.
+    if (tid == 32 && a.prefetch_distance > 0) {
+        const int nx = (int)gridDim.x;
+        int t = (int)blockIdx.x + a.prefetch_distance, bb = b;
+        while (t >= nx) { t -= nx; ++bb; }
+        if (bb < (int)gridDim.y) {
+#pragma unroll 1
+            for (int r0 = 0; r0 < N; r0 += kTmaBoxRows) tma_prefetch_3d(&tmap, t * W * 2, r0, bb);
+        }
+    }
+    mbar_wait(&full_bar, 0);
+
+    C v[16];
+#pragma unroll
+    for (int r = 0; r < 16; ++r) {
+        const uint32_t off = (uint32_t)((j + r * TL) * ROW_BYTES + g * ES);
+        v[r] = *reinterpret_cast<const C *>(tile + tile_swizzle<ROW_BYTES>(off));
+    }
+    __syncthreads();                                 // the landing zone becomes exchange space
+
+    if (a.pre != nullptr) {
+        const C *p = a.pre + (size_t)b * N;
+#pragma unroll
+        for (int r = 0; r < 16; ++r) v[r] = cmul(v[r], ldg_c(p + j + r * TL));
+    }
+    if constexpr (MODE == MODE_INV) fft_line<T, N, +1, false, W, GT>(v, buf, g, j, a.tw, 1 + g);
+    else                            fft_line<T, N, -1, false, W, GT>(v, buf, g, j, a.tw, 1 + g);
+    if (a.mid != nullptr) {
+        const C *m = a.mid + (size_t)b * N;
+#pragma unroll
+        for (int r = 0; r < 16; ++r) v[r] = cmul(v[r], ldg_c(m + j + r * TL));
+    }
+    if constexpr (MODE == MODE_CONV) fft_line<T, N, +1, false, W, GT>(v, buf, g, j, a.tw, 1 + g);
+    if (a.scale != (T)1) {
+#pragma unroll
+        for (int r = 0; r < 16; ++r) { v[r].x *= a.scale; v[r].y *= a.scale; }
+    }
+
+    __syncthreads();                                 // every group is done with its exchange buffer
+#pragma unroll
+    for (int r = 0; r < 16; ++r) {
+        const uint32_t off = (uint32_t)((j + r * TL) * ROW_BYTES + g * ES);
+        *reinterpret_cast<C *>(tile + tile_swizzle<ROW_BYTES>(off)) = v[r];
+    }
+    fence_async_proxy();
+    __syncthreads();
+    if (tid == 0) {
+#pragma unroll 1
+        for (int r0 = 0; r0 < N; r0 += kTmaBoxRows)
+            tma_store_3d(&tmap, tile + (size_t)r0 * ROW_BYTES, col0 * 2, r0, b);
+        tma_store_commit_and_wait();
+    }
+}
+
+// columns per tile for the TMA column pass
+__host__ __device__ constexpr int fr_tma_cols(int N, int elem_bytes)
+{
+    const int TL = N / 16;
+    if (elem_bytes == 16) {
+#ifdef FR_TMAW_F64
+        if (FR_TMAW_F64 * TL <= 512) return FR_TMAW_F64;
+#endif
+        return N <= 1024 ? 4 : (N <= 2048 ? 2 : 1);       // >= 2 resident CTAs per SM wherever the tile allows
+    }
+#ifdef FR_TMAW_F32
+    if (FR_TMAW_F32 * TL <= 1024) return FR_TMAW_F32;
+#endif
+    return N <= 1024 ? 8 : (N <= 2048 ? 4 : 2);
+}
+
+template <typename T, int N> struct ColTmaGeom {
+    static constexpr int TL = N / 16;
+    static constexpr int ES = (int)sizeof(typename cplx_of<T>::type);
+    static constexpr int W = fr_tma_cols(N, ES);
+    static constexpr int threads = W * TL;
+    static constexpr size_t smem = (size_t)W * fr_padded_len(N) * ES;
+    static constexpr int regs_goal = sizeof(T) == 8 ? FR_REGS_F64 : FR_REGS_F32;
+    static constexpr int minb_regs = 65536 / (threads * regs_goal);
+    static constexpr int minb_smem = (int)((226 * 1024) / (smem + 1024));
+    static constexpr int minb0 = minb_regs < minb_smem ? minb_regs : minb_smem;
+    static constexpr int MINB = minb0 < 1 ? 1 : (minb0 > 8 ? 8 : minb0);
+    static constexpr bool supported = TL >= 32;      // named barriers work on whole warps
+};
+
+template <typename T, int N, int MODE>
+cudaError_t launch_col_tma(const PassArgs<T> &a, const CUtensorMap &tmap, int batch, cudaStream_t stream)
+{
+    using G = ColTmaGeom<T, N>;
+    if constexpr (!G::supported) {
+        return cudaErrorNotSupported;
+    } else {
+        auto kern = col_tma_kernel<T, N, G::W, MODE, G::MINB>;
+        static bool configured = false;
+        if (!configured) {
+            cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::smem + 1024);
+            if (e != cudaSuccess) return e;
+            configured = true;
+        }
+        dim3 grid(N / G::W, batch, 1);
+        PassArgs<T> b = a;
+        if (b.prefetch_distance < 0) b.prefetch_distance = -b.prefetch_distance * G::MINB;
+        kern<<<grid, G::threads, G::smem + 1024, stream>>>(b, tmap);
+        return cudaGetLastError();
+    }
+}
+
+} // namespace fresnel

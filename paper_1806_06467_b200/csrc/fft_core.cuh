@@ -179,10 +179,20 @@ template <int N, bool COL, int W> FR_DEV int fr_slot(int p, int line)
 
 template <typename C> FR_DEV C ldg_c(const C *p) { return __ldg(p); }
 
+// Barrier among the threads that share one exchange buffer.  GT = 0: the whole CTA;
+// GT = 32: one warp; otherwise a named barrier over GT threads (id 1..15) so that the line
+// groups of a CTA run independently of one another.
+template <int GT> FR_DEV void fr_sync(int bar_id)
+{
+    if constexpr (GT == 0) __syncthreads();
+    else if constexpr (GT == 32) __syncwarp();
+    else asm volatile("bar.sync %0, %1;" ::"r"(bar_id), "n"(GT) : "memory");
+}
+
 // One Stockham stage on the 16 registers of this thread.  STAGE is 0-based.
-template <typename T, int N, int STAGE, int DIR, bool COL, int W>
+template <typename T, int N, int STAGE, int DIR, bool COL, int W, int GT = 0>
 FR_DEV void fft_stage(typename cplx_of<T>::type (&v)[16], typename cplx_of<T>::type *buf, int line, int j,
-                      const typename cplx_of<T>::type *__restrict__ tw)
+                      const typename cplx_of<T>::type *__restrict__ tw, int bar_id = 0)
 {
     using C = typename cplx_of<T>::type;
     constexpr int TL = N / 16;
@@ -246,7 +256,7 @@ FR_DEV void fft_stage(typename cplx_of<T>::type (&v)[16], typename cplx_of<T>::t
 #pragma unroll
             for (int q = 0; q < 16; ++q) buf[fr_slot<N, COL, W>(p0 + q * (NS + NS / 16), line)] = v[q];
         }
-        __syncthreads();
+        fr_sync<GT>(bar_id);
         if constexpr (TL % 16 == 0) {
             const int p0 = fr_pad(j);
 #pragma unroll
@@ -255,20 +265,20 @@ FR_DEV void fft_stage(typename cplx_of<T>::type (&v)[16], typename cplx_of<T>::t
 #pragma unroll
             for (int r = 0; r < 16; ++r) v[r] = buf[fr_slot<N, COL, W>(fr_pad(j + r * TL), line)];
         }
-        __syncthreads();
+        fr_sync<GT>(bar_id);
     }
 }
 
 // Whole transform of one line: v in, v out, both in the (thread j, register r) <-> j + r*N/16 layout.
-template <typename T, int N, int DIR, bool COL, int W>
+template <typename T, int N, int DIR, bool COL, int W, int GT = 0>
 FR_DEV void fft_line(typename cplx_of<T>::type (&v)[16], typename cplx_of<T>::type *buf, int line, int j,
-                     const typename cplx_of<T>::type *__restrict__ tw)
+                     const typename cplx_of<T>::type *__restrict__ tw, int bar_id = 0)
 {
     constexpr int S = fr_num_stages(N);
-    fft_stage<T, N, 0, DIR, COL, W>(v, buf, line, j, tw);
-    if constexpr (S > 1) fft_stage<T, N, 1, DIR, COL, W>(v, buf, line, j, tw);
-    if constexpr (S > 2) fft_stage<T, N, 2, DIR, COL, W>(v, buf, line, j, tw);
-    if constexpr (S > 3) fft_stage<T, N, 3, DIR, COL, W>(v, buf, line, j, tw);
+    fft_stage<T, N, 0, DIR, COL, W, GT>(v, buf, line, j, tw, bar_id);
+    if constexpr (S > 1) fft_stage<T, N, 1, DIR, COL, W, GT>(v, buf, line, j, tw, bar_id);
+    if constexpr (S > 2) fft_stage<T, N, 2, DIR, COL, W, GT>(v, buf, line, j, tw, bar_id);
+    if constexpr (S > 3) fft_stage<T, N, 3, DIR, COL, W, GT>(v, buf, line, j, tw, bar_id);
 }
 
 } // namespace fresnel

@@ -20,6 +20,17 @@ static cudaError_t by_mode(int mode, const PassArgs<T> &a, int batch, cudaStream
     return cudaErrorInvalidValue;
 }
 
+template <typename T>
+static cudaError_t tma_by_mode(int mode, const PassArgs<T> &a, const CUtensorMap &m, int batch, cudaStream_t s)
+{
+    switch (mode) {
+    case MODE_FWD:  return launch_col_tma<T, FR_N, MODE_FWD>(a, m, batch, s);
+    case MODE_INV:  return launch_col_tma<T, FR_N, MODE_INV>(a, m, batch, s);
+    case MODE_CONV: return launch_col_tma<T, FR_N, MODE_CONV>(a, m, batch, s);
+    }
+    return cudaErrorInvalidValue;
+}
+
 #define FR_CAT2(a, b) a##b
 #define FR_CAT(a, b) FR_CAT2(a, b)
 
@@ -31,5 +42,17 @@ cudaError_t FR_CAT(launch_pass_f64_, FR_N)(bool col, int mode, const PassArgs<do
 {
     return col ? by_mode<double, true>(mode, a, batch, s) : by_mode<double, false>(mode, a, batch, s);
 }
+
+cudaError_t FR_CAT(launch_col_tma_f32_, FR_N)(int mode, const PassArgs<float> &a, const CUtensorMap &m, int batch, cudaStream_t s)
+{
+    return tma_by_mode<float>(mode, a, m, batch, s);
+}
+cudaError_t FR_CAT(launch_col_tma_f64_, FR_N)(int mode, const PassArgs<double> &a, const CUtensorMap &m, int batch, cudaStream_t s)
+{
+    return tma_by_mode<double>(mode, a, m, batch, s);
+}
+// columns per TMA tile (0: this N uses the per-thread-load column pass)
+int FR_CAT(col_tma_width_f32_, FR_N)() { return ColTmaGeom<float, FR_N>::supported ? ColTmaGeom<float, FR_N>::W : 0; }
+int FR_CAT(col_tma_width_f64_, FR_N)() { return ColTmaGeom<double, FR_N>::supported ? ColTmaGeom<double, FR_N>::W : 0; }
 
 } // namespace fresnel

@@ -11,6 +11,7 @@
 // over columns (H is separable); fft2d and direct Fresnel are MODE_FWD/MODE_INV over rows then
 // columns.  Shifts are folded into the tables ((-1)^n signs) and never touch memory.
 #pragma once
+#include <cstdint>
 #include "fft_core.cuh"
 
 namespace fresnel {
@@ -27,7 +28,14 @@ template <typename T> struct PassArgs {
     const T *opd;             // [N][N] or nullptr (row pass only)
     const double *inv_lambda; // [batch] 1/lambda (only read when opd != nullptr)
     T scale;                  // applied last when != 1
+    int prefetch_distance;    // tiles ahead to prefetch into L2 (0: off); ~ number of resident CTAs
 };
+
+// bulk L2 prefetch of a contiguous range (bytes: multiple of 16)
+FR_DEV void l2_prefetch_bulk(const void *p, uint32_t bytes)
+{
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
+}
 
 // exp(2 pi i u) for a phase u given in turns (optic phasor; |u| is typically << 1)
 FR_DEV double2 phasor_turns(double u)
@@ -63,6 +71,20 @@ __global__ void __launch_bounds__(W *(N / 16), MINB) pass_kernel(PassArgs<T> a)
 #pragma unroll
     for (int r = 0; r < 16; ++r) v[r] = g[(size_t)(j + r * TL) * gstride];
 
+    if constexpr (!COL) {
+        // L2 prefetch of the rows (and map rows) a later CTA will load: one bulk request per row
+        if (j == 0 && a.prefetch_distance > 0) {
+            const int nx = (int)gridDim.x;
+            int t = (int)blockIdx.x + a.prefetch_distance, bb = b;
+            while (t >= nx) { t -= nx; ++bb; }
+            if (bb < (int)gridDim.y) {
+                const size_t row = (size_t)t * W + line;
+                l2_prefetch_bulk(a.wf + (size_t)bb * N * N + row * N, (uint32_t)(N * sizeof(C)));
+                if (a.opd != nullptr) l2_prefetch_bulk(a.opd + row * N, (uint32_t)(N * sizeof(T)));
+                if (a.amp != nullptr) l2_prefetch_bulk(a.amp + row * N, (uint32_t)(N * sizeof(T)));
+            }
+        }
+    }
     if constexpr (!COL) {
         if (a.opd != nullptr) {
             const T il = (T)a.inv_lambda[b];
@@ -170,7 +192,9 @@ cudaError_t launch_pass(const PassArgs<T> &a, int batch, cudaStream_t stream)
         configured = true;
     }
     dim3 grid(N / G::W, batch, 1);
-    kern<<<grid, G::threads, G::smem, stream>>>(a);
+    PassArgs<T> b = a;
+    if (b.prefetch_distance < 0) b.prefetch_distance = -b.prefetch_distance * G::MINB;
+    kern<<<grid, G::threads, G::smem, stream>>>(b);
     return cudaGetLastError();
 }
 

@@ -74,5 +74,17 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
+def build_microbench() -> str:
+    """The stand-alone measurement tool of csrc/microbench.cu (profiles/r01_microbench.txt)."""
+    out = os.path.join(HERE, "microbench")
+    cmd = [_nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-o", out,
+           os.path.join(CSRC, "microbench.cu")]
+    subprocess.run(cmd, check=True)
+    return out
+
+
 if __name__ == "__main__":
-    build(force="--force" in sys.argv, verbose=True)
+    if "--microbench" in sys.argv:
+        print("built", build_microbench())
+    else:
+        build(force="--force" in sys.argv, verbose=True)

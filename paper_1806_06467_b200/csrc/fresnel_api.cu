@@ -20,7 +20,7 @@ using namespace fresnel;
 
 namespace {
 
-constexpr int kSlots = 8;               // cached chirp tables per plan
+constexpr int kSlots = 64;              // cached chirp tables per plan (a 20-surface train needs 40)
 const long double PI_L = 3.14159265358979323846264338327950288419716939937510L;
 
 struct TableSlot {

@@ -189,10 +189,11 @@ template <int GT> FR_DEV void fr_sync(int bar_id)
     else asm volatile("bar.sync %0, %1;" ::"r"(bar_id), "n"(GT) : "memory");
 }
 
-// One Stockham stage on the 16 registers of this thread.  STAGE is 0-based.
-template <typename T, int N, int STAGE, int DIR, bool COL, int W, int GT = 0>
-FR_DEV void fft_stage(typename cplx_of<T>::type (&v)[16], typename cplx_of<T>::type *buf, int line, int j,
-                      const typename cplx_of<T>::type *__restrict__ tw, int bar_id = 0)
+// One Stockham stage = compute (twiddles + butterflies, registers only) -> scatter -> barrier ->
+// gather -> barrier.  The three pieces are separate functions so that a kernel can schedule the
+// exchange of one line under the butterflies of another (dual_line.cuh).  STAGE is 0-based.
+template <typename T, int N, int STAGE, int DIR>
+FR_DEV void fft_stage_compute(typename cplx_of<T>::type (&v)[16], int j, const typename cplx_of<T>::type *__restrict__ tw)
 {
     using C = typename cplx_of<T>::type;
     constexpr int TL = N / 16;
@@ -243,28 +244,52 @@ FR_DEV void fft_stage(typename cplx_of<T>::type (&v)[16], typename cplx_of<T>::t
 #pragma unroll
         for (int b = 0; b < B; ++b) dft2<DIR>(v[b], v[b + B]);
     }
+}
+
+// scatter the outputs of stage STAGE (not the last) into the exchange buffer
+template <typename T, int N, int STAGE, bool COL, int W>
+FR_DEV void fft_stage_scatter(const typename cplx_of<T>::type (&v)[16], typename cplx_of<T>::type *buf, int line, int j)
+{
+    constexpr int NS = fr_ns(N, STAGE);
+    const int k = j & (NS - 1);
+    const int base = (j - k) * 16 + k;          // + q*NS ; NS is 1 or a multiple of 16
+    if constexpr (NS == 1) {
+        const int p0 = j * 17;                  // fr_pad(16*j + q) = 17*j + q
+#pragma unroll
+        for (int q = 0; q < 16; ++q) buf[fr_slot<N, COL, W>(p0 + q, line)] = v[q];
+    } else {
+        const int p0 = fr_pad(base);
+#pragma unroll
+        for (int q = 0; q < 16; ++q) buf[fr_slot<N, COL, W>(p0 + q * (NS + NS / 16), line)] = v[q];
+    }
+}
+
+// gather the inputs of the next stage: element j + r*N/16 into register r
+template <typename T, int N, bool COL, int W>
+FR_DEV void fft_stage_gather(typename cplx_of<T>::type (&v)[16], const typename cplx_of<T>::type *buf, int line, int j)
+{
+    constexpr int TL = N / 16;
+    if constexpr (TL % 16 == 0) {
+        const int p0 = fr_pad(j);
+#pragma unroll
+        for (int r = 0; r < 16; ++r) v[r] = buf[fr_slot<N, COL, W>(p0 + r * (TL + TL / 16), line)];
+    } else {
+#pragma unroll
+        for (int r = 0; r < 16; ++r) v[r] = buf[fr_slot<N, COL, W>(fr_pad(j + r * TL), line)];
+    }
+}
+
+template <typename T, int N, int STAGE, int DIR, bool COL, int W, int GT = 0>
+FR_DEV void fft_stage(typename cplx_of<T>::type (&v)[16], typename cplx_of<T>::type *buf, int line, int j,
+                      const typename cplx_of<T>::type *__restrict__ tw, int bar_id = 0)
+{
+    constexpr bool LAST = (STAGE == fr_num_stages(N) - 1);
+    fft_stage_compute<T, N, STAGE, DIR>(v, j, tw);
     // ---- exchange through shared memory (the last stage's output is already in place) ----
     if constexpr (!LAST) {
-        const int k = j & (NS - 1);
-        const int base = (j - k) * 16 + k;          // + q*NS ; NS is 1 or a multiple of 16
-        if constexpr (NS == 1) {
-            const int p0 = j * 17;                  // fr_pad(16*j + q) = 17*j + q
-#pragma unroll
-            for (int q = 0; q < 16; ++q) buf[fr_slot<N, COL, W>(p0 + q, line)] = v[q];
-        } else {
-            const int p0 = fr_pad(base);
-#pragma unroll
-            for (int q = 0; q < 16; ++q) buf[fr_slot<N, COL, W>(p0 + q * (NS + NS / 16), line)] = v[q];
-        }
+        fft_stage_scatter<T, N, STAGE, COL, W>(v, buf, line, j);
         fr_sync<GT>(bar_id);
-        if constexpr (TL % 16 == 0) {
-            const int p0 = fr_pad(j);
-#pragma unroll
-            for (int r = 0; r < 16; ++r) v[r] = buf[fr_slot<N, COL, W>(p0 + r * (TL + TL / 16), line)];
-        } else {
-#pragma unroll
-            for (int r = 0; r < 16; ++r) v[r] = buf[fr_slot<N, COL, W>(fr_pad(j + r * TL), line)];
-        }
+        fft_stage_gather<T, N, COL, W>(v, buf, line, j);
         fr_sync<GT>(bar_id);
     }
 }

@@ -15,7 +15,7 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
-OBJ = os.path.join(HERE, "build")
+OBJ = os.path.join(HERE, "build", os.environ.get("FRESNEL_LIB_NAME", "libfresnel.so").replace(".so", ""))
 # FRESNEL_LIB_NAME / FRESNEL_DEFINES: tuning builds only (e.g. FRESNEL_DEFINES="-DFR_COLW_F64=4")
 LIB = os.path.join(HERE, os.environ.get("FRESNEL_LIB_NAME", "libfresnel.so"))
 EXTRA_DEFINES = os.environ.get("FRESNEL_DEFINES", "").split()
@@ -54,7 +54,7 @@ def _compile(args):
 
 def build(force: bool = False, verbose: bool = False) -> str:
     os.makedirs(OBJ, exist_ok=True)
-    stamp = os.path.join(OBJ, os.path.basename(LIB) + ".digest.txt")
+    stamp = os.path.join(OBJ, "digest.txt")
     digest = _sources_digest()
     if not force and os.path.exists(LIB) and os.path.exists(stamp) and open(stamp).read() == digest:
         return LIB

@@ -11,17 +11,7 @@ namespace fresnel {
     cudaError_t launch_col_tma_f32_##N(int mode, const PassArgs<float> &a, const CUtensorMap &m, int batch, cudaStream_t s);   \
     cudaError_t launch_col_tma_f64_##N(int mode, const PassArgs<double> &a, const CUtensorMap &m, int batch, cudaStream_t s);   \
     int col_tma_width_f32_##N();                                                                                \
-    int col_tma_width_f64_##N();                                                                                \
-    cudaError_t launch_dual_row_f32_##N(int mode, const PassArgs<float> &a, int batch, cudaStream_t s);        \
-    cudaError_t launch_dual_row_f64_##N(int mode, const PassArgs<double> &a, int batch, cudaStream_t s);       \
-    cudaError_t launch_dual_col_f32_##N(int mode, const PassArgs<float> &a, const CUtensorMap &m, int batch, cudaStream_t s);   \
-    cudaError_t launch_dual_col_f64_##N(int mode, const PassArgs<double> &a, const CUtensorMap &m, int batch, cudaStream_t s);  \
-    int dual_width_f32_##N();                                                                                   \
-    int dual_width_f64_##N();                                                                                   \
-    cudaError_t launch_persist_row_f32_##N(int mode, const PassArgs<float> &a, int batch, int sms, cudaStream_t s);   \
-    cudaError_t launch_persist_row_f64_##N(int mode, const PassArgs<double> &a, int batch, int sms, cudaStream_t s);  \
-    int persist_supported_f32_##N();                                                                            \
-    int persist_supported_f64_##N();
+    int col_tma_width_f64_##N();
 FR_DECL(64) FR_DECL(128) FR_DECL(256) FR_DECL(512) FR_DECL(1024) FR_DECL(2048) FR_DECL(4096) FR_DECL(8192)
 #undef FR_DECL
 } // namespace fresnel

@@ -190,20 +190,16 @@ template <int GT> FR_DEV void fr_sync(int bar_id)
 }
 
 // One Stockham stage = compute (twiddles + butterflies, registers only) -> scatter -> barrier ->
-// gather -> barrier.  The three pieces are separate functions so that a kernel can schedule the
-// exchange of one line under the butterflies of another (dual_line.cuh).  STAGE is 0-based.
+// gather -> barrier.  STAGE is 0-based.
+// v[b + q*B] *= w^q, w = W_{Ns*R}^k, k = (j + b*N/16) mod Ns  (none in stage 0: Ns = 1)
 template <typename T, int N, int STAGE, int DIR>
-FR_DEV void fft_stage_compute(typename cplx_of<T>::type (&v)[16], int j, const typename cplx_of<T>::type *__restrict__ tw)
+FR_DEV void fft_stage_twiddle(typename cplx_of<T>::type (&v)[16], int j, const typename cplx_of<T>::type *__restrict__ tw)
 {
     using C = typename cplx_of<T>::type;
     constexpr int TL = N / 16;
     constexpr int R = fr_radix(N, STAGE);
     constexpr int NS = fr_ns(N, STAGE);
     constexpr int B = 16 / R;
-    constexpr bool LAST = (STAGE == fr_num_stages(N) - 1);
-    static_assert(LAST || R == 16, "only the last stage may have a radix below 16");
-
-    // ---- twiddles (none in the first stage: Ns = 1): v[b + q*B] *= w^q, w = W_{Ns*R}^k ----
     if constexpr (STAGE > 0) {
         const C *t = tw + fr_tw_offset(N, STAGE);
 #pragma unroll
@@ -230,7 +226,16 @@ FR_DEV void fft_stage_compute(typename cplx_of<T>::type (&v)[16], int j, const t
             }
         }
     }
-    // ---- butterflies ----
+}
+
+// B = 16/R butterflies of radix R over v[b + q*B], q = 0..R-1
+template <typename T, int N, int STAGE, int DIR>
+FR_DEV void fft_stage_butterfly(typename cplx_of<T>::type (&v)[16])
+{
+    constexpr int R = fr_radix(N, STAGE);
+    constexpr int B = 16 / R;
+    constexpr bool LAST = (STAGE == fr_num_stages(N) - 1);
+    static_assert(LAST || R == 16, "only the last stage may have a radix below 16");
     if constexpr (R == 16) {
         dft16<DIR>(v);
     } else if constexpr (R == 8) {
@@ -244,6 +249,14 @@ FR_DEV void fft_stage_compute(typename cplx_of<T>::type (&v)[16], int j, const t
 #pragma unroll
         for (int b = 0; b < B; ++b) dft2<DIR>(v[b], v[b + B]);
     }
+}
+
+// decimation in time: twiddles on the inputs, then the butterflies
+template <typename T, int N, int STAGE, int DIR>
+FR_DEV void fft_stage_compute(typename cplx_of<T>::type (&v)[16], int j, const typename cplx_of<T>::type *__restrict__ tw)
+{
+    fft_stage_twiddle<T, N, STAGE, DIR>(v, j, tw);
+    fft_stage_butterfly<T, N, STAGE, DIR>(v);
 }
 
 // scatter the outputs of stage STAGE (not the last) into the exchange buffer

@@ -52,11 +52,8 @@ struct fresnel_plan {
     unsigned long long launches = 0;
     int prefetch = 0;                   // L2 prefetch distance in tiles (see pass_kernel.cuh)
     int tma_w = 0;                      // columns per TMA tile of the column pass (0: not used for this N)
-    bool dual = false;                  // dual-line kernels (dual_line.cuh) serve this (N, dtype)
-    bool persist_row = false;           // persistent row pass (persist.cuh)
-    int stagger_ns = 0;
     int sms = 148;
-    CUtensorMap tmap;                   // tensor map of the wavefront last seen by the column pass
+    CUtensorMap tmap{};                  // tensor map of the wavefront last seen by the column pass
     const void *tmap_wf = nullptr;
     cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};   // profiling hook, see fresnel_plan_record_pass_events
     bool ev_armed = false;
@@ -239,26 +236,6 @@ int query_tma_width(int N, fresnel_dtype dt)
     return 0;
 }
 
-int query_persist(int N, fresnel_dtype dt)
-{
-    switch (N) {
-#define FR_CASE(NN) case NN: return dt == FRESNEL_C128 ? persist_supported_f64_##NN() : persist_supported_f32_##NN();
-        FR_CASE(64) FR_CASE(128) FR_CASE(256) FR_CASE(512) FR_CASE(1024) FR_CASE(2048) FR_CASE(4096) FR_CASE(8192)
-#undef FR_CASE
-    }
-    return 0;
-}
-
-int query_dual_width(int N, fresnel_dtype dt)
-{
-    switch (N) {
-#define FR_CASE(NN) case NN: return dt == FRESNEL_C128 ? dual_width_f64_##NN() : dual_width_f32_##NN();
-        FR_CASE(64) FR_CASE(128) FR_CASE(256) FR_CASE(512) FR_CASE(1024) FR_CASE(2048) FR_CASE(4096) FR_CASE(8192)
-#undef FR_CASE
-    }
-    return 0;
-}
-
 // The wavefront as a 3-D tensor {2N scalars, N rows, batch}; a box is {2W scalars, 256 rows, 1}.
 bool make_tensor_map(fresnel_plan *p, void *wf)
 {
@@ -289,23 +266,19 @@ fresnel_status run_pass(fresnel_plan *p, bool col, int mode, void *wf, const voi
 {
     cudaError_t e = cudaErrorInvalidValue;
     const bool tma = col && p->tma_w > 0 && make_tensor_map(p, wf);
-    if (p->dual && col && !tma) return FRESNEL_ERR_CUDA;          // the dual-line column pass has no non-TMA form
     // L2 prefetch of upcoming rows pays when the data does not already sit in the 126 MB L2 (measured:
     // +10..17 % at N >= 4096, -4 % at N = 2048 without maps); TMA tile prefetch of 16..32-byte-wide
     // column boxes costs more TMA issue slots than it saves and stays off.
     const size_t wf_bytes = (size_t)p->batch * p->N * p->N * p->esize();
-    const int prefetch = (!col && (p->persist_row || wf_bytes > ((size_t)64 << 20) || amp || opd)) ? p->prefetch : 0;
+    const int prefetch = (!col && (wf_bytes > ((size_t)64 << 20) || amp || opd)) ? p->prefetch : 0;
     if (p->dtype == FRESNEL_C128) {
         PassArgs<double> a;
         a.wf = (double2 *)wf; a.pre = (const double2 *)pre; a.mid = (const double2 *)mid;
         a.tw = (const double2 *)p->tw; a.amp = (const double *)amp; a.opd = (const double *)opd;
-        a.inv_lambda = p->scal_dev; a.scale = scale; a.prefetch_distance = prefetch; a.stagger_ns = p->stagger_ns;
+        a.inv_lambda = p->scal_dev; a.scale = scale; a.prefetch_distance = prefetch;
         switch (p->N) {
-#define FR_CASE(NN) case NN: e = (p->persist_row && !col) ? launch_persist_row_f64_##NN(mode, a, p->batch, p->sms, p->stream) \
-                               : p->dual ? (col ? launch_dual_col_f64_##NN(mode, a, p->tmap, p->batch, p->stream)   \
-                                                 : launch_dual_row_f64_##NN(mode, a, p->batch, p->stream))          \
-                               : tma ? launch_col_tma_f64_##NN(mode, a, p->tmap, p->batch, p->stream)           \
-                                     : launch_pass_f64_##NN(col, mode, a, p->batch, p->stream); break;
+#define FR_CASE(NN) case NN: e = tma ? launch_col_tma_f64_##NN(mode, a, p->tmap, p->batch, p->stream)           \
+                                   : launch_pass_f64_##NN(col, mode, a, p->batch, p->stream); break;
             FR_CASE(64) FR_CASE(128) FR_CASE(256) FR_CASE(512) FR_CASE(1024) FR_CASE(2048) FR_CASE(4096) FR_CASE(8192)
 #undef FR_CASE
         }
@@ -313,13 +286,10 @@ fresnel_status run_pass(fresnel_plan *p, bool col, int mode, void *wf, const voi
         PassArgs<float> a;
         a.wf = (float2 *)wf; a.pre = (const float2 *)pre; a.mid = (const float2 *)mid;
         a.tw = (const float2 *)p->tw; a.amp = (const float *)amp; a.opd = (const float *)opd;
-        a.inv_lambda = p->scal_dev; a.scale = (float)scale; a.prefetch_distance = prefetch; a.stagger_ns = p->stagger_ns;
+        a.inv_lambda = p->scal_dev; a.scale = (float)scale; a.prefetch_distance = prefetch;
         switch (p->N) {
-#define FR_CASE(NN) case NN: e = (p->persist_row && !col) ? launch_persist_row_f32_##NN(mode, a, p->batch, p->sms, p->stream) \
-                               : p->dual ? (col ? launch_dual_col_f32_##NN(mode, a, p->tmap, p->batch, p->stream)   \
-                                                 : launch_dual_row_f32_##NN(mode, a, p->batch, p->stream))          \
-                               : tma ? launch_col_tma_f32_##NN(mode, a, p->tmap, p->batch, p->stream)           \
-                                     : launch_pass_f32_##NN(col, mode, a, p->batch, p->stream); break;
+#define FR_CASE(NN) case NN: e = tma ? launch_col_tma_f32_##NN(mode, a, p->tmap, p->batch, p->stream)           \
+                                   : launch_pass_f32_##NN(col, mode, a, p->batch, p->stream); break;
             FR_CASE(64) FR_CASE(128) FR_CASE(256) FR_CASE(512) FR_CASE(1024) FR_CASE(2048) FR_CASE(4096) FR_CASE(8192)
 #undef FR_CASE
         }
@@ -410,16 +380,6 @@ fresnel_status fresnel_plan_create(fresnel_plan **out, int N, int batch, fresnel
         p->prefetch = pf ? std::atoi(pf) : -sms;                   // negative: auto = SMs x resident CTAs per SM
     }
     p->tma_w = std::getenv("FRESNEL_NO_TMA") ? 0 : query_tma_width(N, dtype);     // env switch: A/B timing only
-    {
-        const int dw = query_dual_width(N, dtype);
-        const char *du = std::getenv("FRESNEL_DUAL");              // env switch: A/B timing only
-        const bool want = du ? std::atoi(du) != 0 : false;
-        if (dw > 0 && want && encode_tiled_fn() != nullptr) { p->dual = true; p->tma_w = dw; }
-        const char *pe = std::getenv("FRESNEL_PERSIST");           // env switch: A/B timing only
-        p->persist_row = (pe ? std::atoi(pe) != 0 : false) && query_persist(N, dtype) != 0;   // measured slower (r01: 62.8 vs 41.4 us, N=2048 c128): off
-        const char *sg = std::getenv("FRESNEL_STAGGER_NS");
-        p->stagger_ns = sg ? std::atoi(sg) : 0;
-    }
     fresnel_status st = upload_twiddles(p);
     if (st == FRESNEL_OK && cudaMalloc((void **)&p->scal_dev, sizeof(double) * batch) != cudaSuccess) st = FRESNEL_ERR_ALLOC;
     for (int i = 0; i < kSlots && st == FRESNEL_OK; ++i)
@@ -564,7 +524,7 @@ fresnel_status fresnel_surface_as(fresnel_plan *p, void *wf, const double *pixel
     if (st != FRESNEL_OK) return st;
     const void *tl = lens ? p->slots[r[i_lens].slot].dev : nullptr;
     if (!prop) return run_pointwise(p, wf, tl, amp, opd);          // optic only
-    const void *th = std::getenv("FRESNEL_EXP_NOMID") ? nullptr : p->slots[r[i_h].slot].dev;
+    const void *th = p->slots[r[i_h].slot].dev;
     // row pass: optic phasor and x-chirp of the lens on load, FFT, x H1, inverse FFT;
     // column pass: y-chirp of the lens on load, FFT, x H1, inverse FFT
     return run_two_passes(p, MODE_CONV, wf, tl, th, amp, opd, 1.0);

@@ -2,8 +2,6 @@
 // One translation unit per N keeps nvcc parallel and each object small.
 #include "pass_kernel.cuh"
 #include "dispatch.h"
-#include "dual_line.cuh"
-#include "persist.cuh"
 
 #ifndef FR_N
 #error "compile with -DFR_N=<grid size>"
@@ -33,39 +31,6 @@ static cudaError_t tma_by_mode(int mode, const PassArgs<T> &a, const CUtensorMap
     return cudaErrorInvalidValue;
 }
 
-template <typename T>
-static cudaError_t dual_row_by_mode(int mode, const PassArgs<T> &a, int batch, cudaStream_t s)
-{
-    switch (mode) {
-    case MODE_FWD:  return launch_dual_row<T, FR_N, MODE_FWD>(a, batch, s);
-    case MODE_INV:  return launch_dual_row<T, FR_N, MODE_INV>(a, batch, s);
-    case MODE_CONV: return launch_dual_row<T, FR_N, MODE_CONV>(a, batch, s);
-    }
-    return cudaErrorInvalidValue;
-}
-
-template <typename T>
-static cudaError_t dual_col_by_mode(int mode, const PassArgs<T> &a, const CUtensorMap &m, int batch, cudaStream_t s)
-{
-    switch (mode) {
-    case MODE_FWD:  return launch_dual_col<T, FR_N, MODE_FWD>(a, m, batch, s);
-    case MODE_INV:  return launch_dual_col<T, FR_N, MODE_INV>(a, m, batch, s);
-    case MODE_CONV: return launch_dual_col<T, FR_N, MODE_CONV>(a, m, batch, s);
-    }
-    return cudaErrorInvalidValue;
-}
-
-template <typename T>
-static cudaError_t persist_row_by_mode(int mode, const PassArgs<T> &a, int batch, int sms, cudaStream_t s)
-{
-    switch (mode) {
-    case MODE_FWD:  return launch_persist_row<T, FR_N, MODE_FWD>(a, batch, sms, s);
-    case MODE_INV:  return launch_persist_row<T, FR_N, MODE_INV>(a, batch, sms, s);
-    case MODE_CONV: return launch_persist_row<T, FR_N, MODE_CONV>(a, batch, sms, s);
-    }
-    return cudaErrorInvalidValue;
-}
-
 #define FR_CAT2(a, b) a##b
 #define FR_CAT(a, b) FR_CAT2(a, b)
 
@@ -86,35 +51,6 @@ cudaError_t FR_CAT(launch_col_tma_f64_, FR_N)(int mode, const PassArgs<double> &
 {
     return tma_by_mode<double>(mode, a, m, batch, s);
 }
-cudaError_t FR_CAT(launch_dual_row_f32_, FR_N)(int mode, const PassArgs<float> &a, int batch, cudaStream_t s)
-{
-    return dual_row_by_mode<float>(mode, a, batch, s);
-}
-cudaError_t FR_CAT(launch_dual_row_f64_, FR_N)(int mode, const PassArgs<double> &a, int batch, cudaStream_t s)
-{
-    return dual_row_by_mode<double>(mode, a, batch, s);
-}
-cudaError_t FR_CAT(launch_dual_col_f32_, FR_N)(int mode, const PassArgs<float> &a, const CUtensorMap &m, int batch, cudaStream_t s)
-{
-    return dual_col_by_mode<float>(mode, a, m, batch, s);
-}
-cudaError_t FR_CAT(launch_dual_col_f64_, FR_N)(int mode, const PassArgs<double> &a, const CUtensorMap &m, int batch, cudaStream_t s)
-{
-    return dual_col_by_mode<double>(mode, a, m, batch, s);
-}
-cudaError_t FR_CAT(launch_persist_row_f32_, FR_N)(int mode, const PassArgs<float> &a, int batch, int sms, cudaStream_t s)
-{
-    return persist_row_by_mode<float>(mode, a, batch, sms, s);
-}
-cudaError_t FR_CAT(launch_persist_row_f64_, FR_N)(int mode, const PassArgs<double> &a, int batch, int sms, cudaStream_t s)
-{
-    return persist_row_by_mode<double>(mode, a, batch, sms, s);
-}
-int FR_CAT(persist_supported_f32_, FR_N)() { return PersistGeom<float, FR_N>::supported ? 1 : 0; }
-int FR_CAT(persist_supported_f64_, FR_N)() { return PersistGeom<double, FR_N>::supported ? 1 : 0; }
-// columns per TMA tile of the dual-line column pass (0: not available for this N)
-int FR_CAT(dual_width_f32_, FR_N)() { return DualGeom<float, FR_N>::supported ? DualGeom<float, FR_N>::W : 0; }
-int FR_CAT(dual_width_f64_, FR_N)() { return DualGeom<double, FR_N>::supported ? DualGeom<double, FR_N>::W : 0; }
 // columns per TMA tile (0: this N uses the per-thread-load column pass)
 int FR_CAT(col_tma_width_f32_, FR_N)() { return ColTmaGeom<float, FR_N>::supported ? ColTmaGeom<float, FR_N>::W : 0; }
 int FR_CAT(col_tma_width_f64_, FR_N)() { return ColTmaGeom<double, FR_N>::supported ? ColTmaGeom<double, FR_N>::W : 0; }

@@ -29,7 +29,6 @@ template <typename T> struct PassArgs {
     const double *inv_lambda; // [batch] 1/lambda (only read when opd != nullptr)
     T scale;                  // applied last when != 1
     int prefetch_distance;    // tiles ahead to prefetch into L2 (0: off); ~ number of resident CTAs
-    int stagger_ns;           // persistent kernels: start delay between the line groups of a CTA
 };
 
 // bulk L2 prefetch of a contiguous range (bytes: multiple of 16)
@@ -70,11 +69,7 @@ __global__ void __launch_bounds__(W *(N / 16), MINB) pass_kernel(PassArgs<T> a)
 
     C v[16];
 #pragma unroll
-#ifdef FR_EXP_LDCS
-    for (int r = 0; r < 16; ++r) v[r] = __ldcs(&g[(size_t)(j + r * TL) * gstride]);
-#else
     for (int r = 0; r < 16; ++r) v[r] = g[(size_t)(j + r * TL) * gstride];
-#endif
 
     if constexpr (!COL) {
         // L2 prefetch of the rows (and map rows) a later CTA will load: one bulk request per row
@@ -128,11 +123,7 @@ __global__ void __launch_bounds__(W *(N / 16), MINB) pass_kernel(PassArgs<T> a)
         for (int r = 0; r < 16; ++r) { v[r].x *= a.scale; v[r].y *= a.scale; }
     }
 #pragma unroll
-#ifdef FR_EXP_LDCS
-    for (int r = 0; r < 16; ++r) __stcs(&g[(size_t)(j + r * TL) * gstride], v[r]);
-#else
     for (int r = 0; r < 16; ++r) g[(size_t)(j + r * TL) * gstride] = v[r];
-#endif
 }
 
 // ---- launch geometry -------------------------------------------------------------------------------

@@ -77,7 +77,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
 def build_microbench() -> str:
     """The stand-alone measurement tool of csrc/microbench.cu (profiles/r01_microbench.txt)."""
     out = os.path.join(HERE, "microbench")
-    cmd = [_nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-o", out,
+    cmd = [_nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "--expt-relaxed-constexpr", "-o", out,
            os.path.join(CSRC, "microbench.cu")]
     subprocess.run(cmd, check=True)
     return out

@@ -1,11 +1,15 @@
 // microbench.cu -- stand-alone measurements behind DESIGN.md's design decisions (not part of libfresnel.so):
 //   HBM copy bandwidth, row-tile vs column-tile (strided 16/32/64/128-byte segment) in-place copies with
 //   per-thread loads, L2-resident read bandwidth, and the plain-ALU roofs (DFMA / FFMA) that
-//   MEASURED_PEAKS.json does not carry.   Build + run:
+//   MEASURED_PEAKS.json does not carry; and the IN-SM rates of the transform itself (no HBM): the stage code
+//   of fft_core.cuh on registers + shared memory only -- butterflies alone, exchanges alone, both -- in SM
+//   cycles per element, next to a synthetic stream that interleaves DFMA with 128-bit shared-memory traffic
+//   in every warp (what the two pipes can do when nothing orders them).   Build + run:
 //     python -m paper_1806_06467_b200.build --microbench && ./paper_1806_06467_b200/microbench
 #include <cstdio>
 #include <cstdlib>
 #include <cuda_runtime.h>
+#include "fft_core.cuh"
 #define CK(x) do{cudaError_t e=(x); if(e!=cudaSuccess){printf("CUDA error %s at %d\n",cudaGetErrorString(e),__LINE__); exit(1);} }while(0)
 
 __global__ void copy16(const int4* __restrict__ a, int4* __restrict__ b, size_t n){
@@ -72,6 +76,105 @@ template<int SEGE> void run_row(int4* a,int N){
   CK(cudaGetLastError());
   double bytes=2.0*N*(double)N*16; printf("  row N=%d lines=%d threads=%4d: %.3f ms  %.0f GB/s\n",N,SEGE,threads,ms,bytes/ms/1e6);
 }
+// ---- in-SM rates ---------------------------------------------------------------------------------------------
+// VAR 0: forward + inverse transform of a line (the convolution pass without its table multiplies),
+// VAR 1: the butterflies and twiddles of the same stages only, VAR 2: the four exchanges only.
+// G groups of N/16 threads per CTA, one CTA per SM; GTX = 32 replaces the group barriers by __syncwarp
+// (timing only: the bound a warp-local exchange could reach).
+template <typename T, int N, int G, int VAR, int GTX>
+__global__ void __launch_bounds__(G * (N / 16), 1) insm(int iters, const typename fresnel::cplx_of<T>::type* tw, typename fresnel::cplx_of<T>::type* out){
+  using namespace fresnel; using C = typename cplx_of<T>::type;
+  constexpr int TL = N / 16, PL = fr_padded_len(N); constexpr int GT = GTX >= 0 ? GTX : (G == 1 ? 0 : TL);
+  extern __shared__ __align__(16) unsigned char smraw[];
+  const int tid = threadIdx.x, grp = tid / TL, j = tid % TL;
+  C* buf = reinterpret_cast<C*>(smraw) + (size_t)grp * PL;
+  C v[16];
+  #pragma unroll
+  for (int r = 0; r < 16; ++r) { v[r].x = (T)(tid + r) * (T)1e-3; v[r].y = (T)r; }
+  for (int it = 0; it < iters; ++it) {
+    int jj = j; asm volatile("" : "+r"(jj));            // keep address and twiddle arithmetic inside the loop
+    const C* t = tw; asm volatile("" : "+l"(t));
+    if (VAR == 0) {
+      fft_line<T, N, -1, false, 1, GT>(v, buf, 0, jj, t, 1 + grp);
+      asm volatile("" : "+l"(t));
+      fft_line<T, N, +1, false, 1, GT>(v, buf, 0, jj, t, 1 + grp);
+    } else if (VAR == 1) {
+      fft_stage_compute<T, N, 0, -1>(v, jj, t); fft_stage_compute<T, N, 1, -1>(v, jj, t);
+      if constexpr (fr_num_stages(N) > 2) fft_stage_compute<T, N, 2, -1>(v, jj, t);
+      asm volatile("" : "+l"(t));
+      fft_stage_compute<T, N, 0, +1>(v, jj, t); fft_stage_compute<T, N, 1, +1>(v, jj, t);
+      if constexpr (fr_num_stages(N) > 2) fft_stage_compute<T, N, 2, +1>(v, jj, t);
+    } else {
+      #pragma unroll
+      for (int rep = 0; rep < 2; ++rep) {
+        fft_stage_scatter<T, N, 0, false, 1>(v, buf, 0, jj); fr_sync<GT>(1 + grp);
+        fft_stage_gather<T, N, false, 1>(v, buf, 0, jj); fr_sync<GT>(1 + grp);
+        fft_stage_scatter<T, N, 1, false, 1>(v, buf, 0, jj); fr_sync<GT>(1 + grp);
+        fft_stage_gather<T, N, false, 1>(v, buf, 0, jj); fr_sync<GT>(1 + grp);
+      }
+    }
+    #pragma unroll
+    for (int r = 0; r < 16; ++r) { v[r].x *= (T)0.01; v[r].y *= (T)0.01; }
+  }
+  C s = v[0];
+  #pragma unroll
+  for (int r = 1; r < 16; ++r) { s.x += v[r].x; s.y += v[r].y; }
+  out[blockIdx.x * blockDim.x + tid] = s;
+}
+template <typename T, int N, int G, int VAR, int GTX = -1> void run_insm(const char* what, double clock_hz){
+  using C = typename fresnel::cplx_of<T>::type;
+  C *tw, *out; CK(cudaMalloc(&tw, 65536 * sizeof(C))); CK(cudaMemset(tw, 0, 65536 * sizeof(C))); CK(cudaMalloc(&out, 148 * 1024 * sizeof(C)));
+  const int smem = G * fresnel::fr_padded_len(N) * sizeof(C);
+  CK(cudaFuncSetAttribute(insm<T, N, G, VAR, GTX>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+  const int iters = 400;
+  float ms = timeit([&]{ insm<T, N, G, VAR, GTX><<<148, G * (N / 16), smem>>>(iters, tw, out); }, 3);
+  CK(cudaGetLastError());
+  printf("  in-SM %-22s N=%d %s groups/SM=%d: %.3f clk/element/SM\n", what, N, sizeof(T) == 8 ? "f64" : "f32", G, ms * 1e-3 * clock_hz / iters / ((double)G * N));
+  cudaFree(tw); cudaFree(out);
+}
+// every warp interleaves NM*16 DFMA with NX (STS.128 + LDS.128) pairs per iteration, no barriers, thread-private slots
+template <int NM, int NX, int WARPS>
+__global__ void __launch_bounds__(WARPS * 32, 1) overlap(int iters, double* out){
+  extern __shared__ double2 sm2[];
+  const int tid = threadIdx.x;
+  double a[16];
+  #pragma unroll
+  for (int i = 0; i < 16; ++i) a[i] = tid + i;
+  const double b = 1.0000001, c = 0.5;
+  double2 v[8];
+  #pragma unroll
+  for (int i = 0; i < 8; ++i) v[i] = make_double2(tid, i);
+  const unsigned base = (unsigned)__cvta_generic_to_shared(sm2 + tid);
+  for (int it = 0; it < iters; ++it) {
+    #pragma unroll
+    for (int u = 0; u < (NM > NX ? NM : NX); ++u) {
+      if (u < NX) asm volatile("st.shared.v2.f64 [%0], {%1, %2};" ::"r"(base + (u & 7) * WARPS * 32 * 16), "d"(v[u & 7].x), "d"(v[u & 7].y) : "memory");
+      if (u < NM) {
+        #pragma unroll
+        for (int i = 0; i < 16; ++i) a[i] = fma(a[i], b, c);
+      }
+      if (u < NX) asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v[(u + 3) & 7].x), "=d"(v[(u + 3) & 7].y) : "r"(base + ((u + 5) & 7) * WARPS * 32 * 16) : "memory");
+    }
+  }
+  double s = 0;
+  #pragma unroll
+  for (int i = 0; i < 16; ++i) s += a[i];
+  #pragma unroll
+  for (int i = 0; i < 8; ++i) s += v[i].x + v[i].y;
+  out[blockIdx.x * WARPS * 32 + tid] = s;
+}
+template <int NM, int NX, int WARPS> void run_overlap(double clock_hz){
+  double* out; CK(cudaMalloc(&out, 148 * 1024 * 8));
+  const int smem = WARPS * 32 * 8 * 16;
+  CK(cudaFuncSetAttribute(overlap<NM, NX, WARPS>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+  const int iters = 4000;
+  float ms = timeit([&]{ overlap<NM, NX, WARPS><<<148, WARPS * 32, smem>>>(iters, out); }, 3);
+  CK(cudaGetLastError());
+  printf("  overlap warps/SM=%2d dfma=%3d lds+sts=%2d per warp-iteration: %7.1f clk   (fp64 pipe alone %4.0f, shared-memory pipe alone %4.0f)\n",
+         WARPS, NM * 16, NX * 2, ms * 1e-3 * clock_hz / iters, WARPS * NM * 16 * 2.0 / 4, WARPS * NX * 2 * 4.0);
+  cudaFree(out);
+}
+
 int main(){
   cudaDeviceProp p; CK(cudaGetDeviceProperties(&p,0)); printf("%s SMs=%d L2=%d MB clock=%d MHz\n",p.name,p.multiProcessorCount,p.l2CacheSize>>20,p.clockRate/1000);
   size_t n=(size_t)1<<30; // 1 GiB
@@ -91,5 +194,22 @@ int main(){
     double fl=2.0*148*8*256*(double)iters*16*8; printf("DFMA peak: %.3f ms %.2f TFLOP/s\n",ms,fl/ms/1e9); }
   { float* o; CK(cudaMalloc(&o,148*8*256*4)); int iters=4000; float ms=timeit([&]{ fmapeak<float><<<148*8,256>>>(o,iters); },5);
     double fl=2.0*148*8*256*(double)iters*16*8; printf("FFMA peak: %.3f ms %.2f TFLOP/s\n",ms,fl/ms/1e9); }
+  // in-SM rates (cycles at the nominal clock printed above)
+  { const double hz = p.clockRate * 1e3;
+    printf("in-SM (registers + shared memory only; HBM needs %.2f clk/element/SM for complex128, %.2f for complex64 at 6.55 TB/s)\n",
+           32.0 / (6.55e12 / 148 / hz), 16.0 / (6.55e12 / 148 / hz));
+    run_insm<double, 2048, 1, 1>("butterflies", hz); run_insm<double, 2048, 4, 1>("butterflies", hz);
+    run_insm<double, 2048, 1, 2>("exchanges", hz);   run_insm<double, 2048, 4, 2>("exchanges", hz);
+    run_insm<double, 2048, 1, 0>("transform pair", hz); run_insm<double, 2048, 2, 0>("transform pair", hz);
+    run_insm<double, 2048, 3, 0>("transform pair", hz); run_insm<double, 2048, 4, 0>("transform pair", hz);
+    run_insm<double, 2048, 4, 0, 32>("pair, warp-local sync", hz);
+    run_insm<double, 4096, 2, 1>("butterflies", hz); run_insm<double, 4096, 2, 2>("exchanges", hz); run_insm<double, 4096, 2, 0>("transform pair", hz);
+    run_insm<double, 4096, 2, 0, 32>("pair, warp-local sync", hz);
+    run_insm<float, 2048, 4, 1>("butterflies", hz); run_insm<float, 2048, 4, 2>("exchanges", hz);
+    run_insm<float, 2048, 4, 0>("transform pair", hz); run_insm<float, 2048, 8, 0>("transform pair", hz);
+    run_insm<float, 2048, 8, 0, 32>("pair, warp-local sync", hz);
+    run_insm<float, 4096, 4, 1>("butterflies", hz); run_insm<float, 4096, 4, 2>("exchanges", hz); run_insm<float, 4096, 4, 0>("transform pair", hz);
+    run_overlap<8, 0, 16>(hz); run_overlap<0, 8, 16>(hz); run_overlap<8, 8, 16>(hz); run_overlap<8, 8, 4>(hz);
+  }
   return 0;
 }

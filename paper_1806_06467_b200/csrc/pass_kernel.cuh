@@ -37,18 +37,73 @@ FR_DEV void l2_prefetch_bulk(const void *p, uint32_t bytes)
     asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
 }
 
-// exp(2 pi i u) for a phase u given in turns (optic phasor; |u| is typically << 1)
-FR_DEV double2 phasor_turns(double u)
+// exp(2 pi i u) for a phase u given in turns (optic phasor, Eq. 3).  Surface maps are a small fraction of a
+// wave, so the common case |u| <= 1/8 is a pair of Taylor polynomials in u^2 with coefficients (2 pi)^n / n!
+// (truncation < 1e-19 double, < 3e-9 float): no range reduction, no quadrant logic, no branch.  Larger phases
+// go through phasor_turns_any (out of line, so that the common path stays small).
+FR_DEV double2 phasor_turns_small(double u)
+{
+    const double t = u * u;
+    double s = 0.1042291622081398411727104, c = 0.2820059684557912150702702;
+    s = fma(s, t, -0.7181223017785005122317403);  c = fma(c, t, -1.714390711088672065421586);
+    s = fma(s, t, 3.819952584848282127733792);    c = fma(c, t, 7.903536371318468804212103);
+    s = fma(s, t, -15.09464257682299039182662);   c = fma(c, t, -26.42625678337439745290065);
+    s = fma(s, t, 42.05869394489765314498681);    c = fma(c, t, 60.24464137187666036272111);
+    s = fma(s, t, -76.70585975306138584163064);   c = fma(c, t, -85.45681720669372773601951);
+    s = fma(s, t, 81.60524927607505420339768);    c = fma(c, t, 64.93939402266829149096022);
+    s = fma(s, t, -41.34170224039976023396842);   c = fma(c, t, -19.73920880217871723766898);
+    s = fma(s, t, 6.283185307179586476925287);    c = fma(c, t, 1.0);
+    return make_double2(c, s * u);
+}
+FR_DEV float2 phasor_turns_small(float u)
+{
+    const float t = u * u;
+    float s = -15.09464257682299039182662f, c = -26.42625678337439745290065f;
+    s = fmaf(s, t, 42.05869394489765314498681f);   c = fmaf(c, t, 60.24464137187666036272111f);
+    s = fmaf(s, t, -76.70585975306138584163064f);  c = fmaf(c, t, -85.45681720669372773601951f);
+    s = fmaf(s, t, 81.60524927607505420339768f);   c = fmaf(c, t, 64.93939402266829149096022f);
+    s = fmaf(s, t, -41.34170224039976023396842f);  c = fmaf(c, t, -19.73920880217871723766898f);
+    s = fmaf(s, t, 6.283185307179586476925287f);   c = fmaf(c, t, 1.0f);
+    return make_float2(c, s * u);
+}
+static __device__ __noinline__ double2 phasor_turns_any(double u)
 {
     double s, c;
     sincospi(2.0 * u, &s, &c);
     return make_double2(c, s);
 }
-FR_DEV float2 phasor_turns(float u)
+static __device__ __noinline__ float2 phasor_turns_any(float u)
 {
     float s, c;
     sincospif(2.0f * u, &s, &c);
     return make_float2(c, s);
+}
+FR_DEV bool phasor_is_small(double u) { return fabs(u) <= 0.125; }
+FR_DEV bool phasor_is_small(float u) { return fabsf(u) <= 0.125f; }
+template <typename T> FR_DEV typename cplx_of<T>::type phasor_turns(T u)
+{
+    return phasor_is_small(u) ? phasor_turns_small(u) : phasor_turns_any(u);
+}
+
+// v[r] *= exp(2 pi i * opd[r*stride] * inv_lambda), r = 0..15: polynomial for all sixteen, then the rare
+// large phases one by one
+template <typename T>
+FR_DEV void apply_opd16(typename cplx_of<T>::type (&v)[16], const T *__restrict__ o, int stride, T inv_lambda)
+{
+    T u[16];
+    bool all_small = true;
+#pragma unroll
+    for (int r = 0; r < 16; ++r) {
+        u[r] = o[r * stride] * inv_lambda;
+        all_small = all_small && phasor_is_small(u[r]);
+    }
+    if (all_small) {
+#pragma unroll
+        for (int r = 0; r < 16; ++r) v[r] = cmul(v[r], phasor_turns_small(u[r]));
+    } else {
+#pragma unroll
+        for (int r = 0; r < 16; ++r) v[r] = cmul(v[r], phasor_turns_any(u[r]));
+    }
 }
 
 template <typename T, int N, bool COL, int W, int MODE, int MINB>
@@ -87,10 +142,7 @@ __global__ void __launch_bounds__(W *(N / 16), MINB) pass_kernel(PassArgs<T> a)
     }
     if constexpr (!COL) {
         if (a.opd != nullptr) {
-            const T il = (T)a.inv_lambda[b];
-            const T *o = a.opd + (size_t)idx * N;
-#pragma unroll
-            for (int r = 0; r < 16; ++r) v[r] = cmul(v[r], phasor_turns(o[j + r * TL] * il));
+            apply_opd16<T>(v, a.opd + (size_t)idx * N + j, TL, (T)a.inv_lambda[b]);
         }
         if (a.amp != nullptr) {
             const T *m = a.amp + (size_t)idx * N;

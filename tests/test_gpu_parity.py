@@ -165,6 +165,28 @@ def test_surface_as_fused_vs_oracle_and_primitives(torch_cuda, B, oracle, N, dty
     assert rel_batch(g.cpu().numpy(), want0) <= TOL[dtype]
 
 
+@pytest.mark.parametrize("dtype", ["c128", "c64"])
+def test_mask_large_opd_both_phasor_branches(torch_cuda, B, oracle, dtype):
+    """Eq. 3 with an OPD of several waves: the kernel's small-phase polynomial (|OPD/lambda| <= 1/8) and
+    its library branch are both taken, stand-alone and fused into the row pass."""
+    from paper_1806_06467_b200 import inputs
+    N = 512
+    u = field(N, 911, 1, dtype)
+    lam, dx = np.array([600e-9]), np.array([1e-5])
+    opd = inputs.psd_map(N, 1e-5, 2.5, 400e-9, 912)             # RMS 2/3 wave: |u| spans 0 .. ~3 turns
+    assert (np.abs(opd / lam[0]) > 0.125).mean() > 0.3 and (np.abs(opd / lam[0]) <= 0.125).mean() > 0.05
+    plan = B.Plan(N, 1, dtype)
+    do = map_dev(torch_cuda, opd, dtype)
+    d = to_dev(torch_cuda, u, dtype)
+    plan.apply_mask(d, None, do, lam)
+    want = oracle.apply_mask(u[0], None, map_host(opd, dtype), lam[0])[None]
+    assert rel_batch(d.cpu().numpy(), want) <= TOL[dtype]
+    d = to_dev(torch_cuda, u, dtype)
+    plan.surface_as(d, dx, lam, None, None, do, 0.02)
+    want = oracle.surface_as_batch(u, dx, lam, None, None, map_host(opd, dtype), 0.02)
+    assert rel_batch(d.cpu().numpy(), want) <= TOL[dtype]
+
+
 def test_config1(torch_cuda, B, oracle):
     from paper_1806_06467_b200 import inputs
     wl = inputs.config1()

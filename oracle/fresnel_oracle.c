@@ -360,3 +360,18 @@ int oracle_surface_as(double *u, int N, double dx, double lambda, double f,
     if ((amp || opd) && (rc = oracle_apply_mask(u, N, amp, opd, lambda)) != ORACLE_OK) return rc;
     return oracle_propagate_as(u, N, dx, lambda, z);
 }
+
+/* ---- broadband (polychromatic) image: incoherent sum over wavelengths ------------------------------
+ * "calculations must be repeated for all of the wavelengths" (one process per wavelength,
+ * PAPER.md:63): a broadband image is the weighted sum of the monochromatic intensities,
+ *     image[j][k] += w * |u[j][k]|^2        (one call per wavelength).
+ * u: N x N interleaved complex, image: N x N real, both host. */
+int oracle_accumulate_intensity(const double *u, int N, double w, double *image)
+{
+    if (!u || !image || N <= 0) return ORACLE_ERR_INVALID_ARG;
+    for (long i = 0; i < (long)N * N; ++i) {
+        const double re = u[2 * i], im = u[2 * i + 1];
+        image[i] += w * (re * re + im * im);
+    }
+    return ORACLE_OK;
+}

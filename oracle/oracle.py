@@ -42,6 +42,8 @@ def lib():
         L.oracle_propagate_direct.argtypes = [dp, ctypes.c_int, dp, ctypes.c_double, ctypes.c_double]
         L.oracle_surface_as.argtypes = [dp, ctypes.c_int, ctypes.c_double, ctypes.c_double, ctypes.c_double,
                                         dp, dp, ctypes.c_double]
+        L.oracle_accumulate_intensity.argtypes = [dp, ctypes.c_int, ctypes.c_double, dp]
+        L.oracle_accumulate_intensity.restype = ctypes.c_int
         for name in ("oracle_dft2_naive", "oracle_fft2", "oracle_fftshift", "oracle_ifftshift", "oracle_fft2d",
                      "oracle_apply_qpf", "oracle_apply_mask", "oracle_propagate_as", "oracle_propagate_direct",
                      "oracle_surface_as"):
@@ -166,3 +168,22 @@ def surface_as_batch(u, dx, lam, f, amp, opd, z):
     u = np.asarray(u)
     return np.stack([surface_as(u[b], _per_batch(dx, b), _per_batch(lam, b), f, amp, opd, z)
                      for b in range(u.shape[0])])
+
+
+def accumulate_intensity(u, w, image=None):
+    """image += w * |u|^2 (NEXT-3).  u: (N, N) complex; returns the (N, N) float64 image."""
+    a = np.ascontiguousarray(np.asarray(u, dtype=np.complex128))
+    N = a.shape[-1]
+    img = np.zeros((N, N)) if image is None else np.ascontiguousarray(np.asarray(image, dtype=np.float64)).copy()
+    _check(lib().oracle_accumulate_intensity(_dptr(a), N, float(w), img.ctypes.data_as(ctypes.POINTER(ctypes.c_double))),
+           "accumulate_intensity")
+    return img
+
+
+def broadband_image(u, weights):
+    """sum_b weights[b] * |u[b]|^2 for a (batch, N, N) stack of monochromatic fields."""
+    u = np.asarray(u)
+    img = np.zeros(u.shape[-2:])
+    for b in range(u.shape[0]):
+        img = accumulate_intensity(u[b], float(np.asarray(weights)[b]), img)
+    return img

@@ -374,3 +374,39 @@ def test_oracle_rejects_bad_arguments(oracle):
         oracle.propagate_as(u, -1e-5, 1e-6, 0.1)
     with pytest.raises(oracle.OracleError):
         oracle.dft2_naive(rnd(128, 1), -1)
+
+
+# ---- P14: broadband image ("repeated for all of the wavelengths") ----
+def test_p14_accumulate_intensity_closed_forms(oracle):
+    N = 64
+    img0 = np.full((N, N), 2.0)
+    u = np.full((N, N), 3 + 4j)
+    assert np.array_equal(oracle.accumulate_intensity(u, 0.5, img0), np.full((N, N), 14.5))      # 2 + 0.5*25, exact
+    assert np.array_equal(img0, np.full((N, N), 2.0))                                           # caller's image untouched
+    v = rnd(N, 21)
+    assert np.array_equal(oracle.accumulate_intensity(v, 0.0, img0), img0)                      # zero weight
+    one = oracle.accumulate_intensity(v, 1.0)
+    assert rel(one, v.real ** 2 + v.imag ** 2) <= 1e-16
+    assert rel(oracle.accumulate_intensity(v, 0.25, one), 1.25 * one) <= 1e-15                  # linear in the weight
+    # a pure phase factor does not change the image
+    assert rel(oracle.accumulate_intensity(v * np.exp(0.7j), 1.0), one) <= 1e-15
+
+
+def test_p14_broadband_energy_and_gaussian_beam_intensity(oracle):
+    """Two wavelengths of the same Gaussian waist: sum_b w_b |U_b|^2 after propagation equals
+    sum_b w_b (w0/w_b(z))^2 exp(-2 r^2 / w_b(z)^2), w_b(z) = w0 sqrt(1 + (z/zR_b)^2), and carries the
+    weighted input energy (Parseval per wavelength)."""
+    N, dx, w0, z = 512, 4e-5, 2e-3, 1.5
+    lams, wts = np.array([500e-9, 1000e-9]), np.array([0.3, 0.7])
+    x = (np.arange(N) - N // 2) * dx
+    r2 = x[None, :] ** 2 + x[:, None] ** 2
+    u0 = np.exp(-r2 / w0 ** 2).astype(np.complex128)
+    stack = np.stack([oracle.propagate_as(u0, dx, lam, z) for lam in lams])
+    img = oracle.broadband_image(stack, wts)
+    want = np.zeros((N, N))
+    for lam, wt in zip(lams, wts):
+        zr = np.pi * w0 ** 2 / lam
+        wz = w0 * np.sqrt(1 + (z / zr) ** 2)
+        want += wt * (w0 / wz) ** 2 * np.exp(-2 * r2 / wz ** 2)
+    assert rel(img, want) <= 1e-9
+    assert abs(img.sum() / (wts.sum() * (np.abs(u0) ** 2).sum()) - 1) <= 1e-13

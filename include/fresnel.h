@@ -123,6 +123,18 @@ fresnel_status fresnel_propagate_direct(fresnel_plan *p, void *wf, double *pixel
 fresnel_status fresnel_surface_as(fresnel_plan *p, void *wf, const double *pixel, const double *lambda,
                                   double f, const void *amp, const void *opd, double z);
 
+/* Broadband (polychromatic) image: the incoherent, weighted sum of the batch's monochromatic intensities
+ * ("calculations must be repeated for all of the wavelengths"; one process per wavelength in
+ * the paper):
+ *     image[j][k] += sum_b weight[b] * |wf[b][j][k]|^2
+ * wf: device, [batch][N][N] complex of the plan's dtype, read only.  image: device, real [N][N] of the
+ * matching precision (double for C128, float for C64), accumulated in place (zero it first for a fresh
+ * image); the sum over the batch is formed in double.  weight: HOST array of length batch (consumed
+ * before return; non-finite values: FRESNEL_ERR_INVALID_ARG).  One pass: reads the batch once, the image
+ * once, writes the image once.  With the batch sharded over GPUs each rank accumulates its own image and
+ * one sum-reduction of N*N reals finishes the job (paper_1806_06467_b200/sharding.py). */
+fresnel_status fresnel_accumulate_intensity(fresnel_plan *p, const void *wf, const double *weight, void *image);
+
 /* ---- host <-> device staging on the plan's stream (used by the end-to-end benchmark) ---------- */
 
 /* Asynchronous copies ordered with the plan's work.  `host` should be pinned for real overlap. */

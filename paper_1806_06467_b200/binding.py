@@ -28,7 +28,7 @@ C64, C128 = 0, 1
 SYMBOLS = (
     "fresnel_plan_create", "fresnel_plan_set_stream", "fresnel_plan_synchronize", "fresnel_plan_destroy",
     "fresnel_plan_launch_count", "fresnel_plan_record_pass_events", "fresnel_apply_qpf", "fresnel_apply_mask", "fresnel_fft2d",
-    "fresnel_propagate_as", "fresnel_propagate_direct", "fresnel_surface_as", "fresnel_memcpy_h2d",
+    "fresnel_propagate_as", "fresnel_propagate_direct", "fresnel_surface_as", "fresnel_accumulate_intensity", "fresnel_memcpy_h2d",
     "fresnel_memcpy_d2h", "fresnel_status_string", "fresnel_version",
 )
 
@@ -64,6 +64,7 @@ def lib() -> ctypes.CDLL:
     L.fresnel_propagate_as.argtypes = [vp, vp, dp, dp, cd]
     L.fresnel_propagate_direct.argtypes = [vp, vp, dp, dp, cd]
     L.fresnel_surface_as.argtypes = [vp, vp, dp, dp, cd, vp, vp, cd]
+    L.fresnel_accumulate_intensity.argtypes = [vp, vp, dp, vp]
     L.fresnel_memcpy_h2d.argtypes = [vp, vp, vp, ctypes.c_size_t]
     L.fresnel_memcpy_d2h.argtypes = [vp, vp, vp, ctypes.c_size_t]
     for s in SYMBOLS:
@@ -192,6 +193,11 @@ class Plan:
         ff = math.inf if f is None else float(f)
         self._chk(lib().fresnel_surface_as(self._h, self._wf(wf), pp, lp, ff, self._map(amp), self._map(opd), float(z)),
                   "fresnel_surface_as")
+
+    def accumulate_intensity(self, wf, weight, image) -> None:
+        """image += sum_b weight[b] * |wf[b]|^2 (image: real N x N device tensor of the plan's precision)."""
+        _, wp = _darr(weight, self.batch)
+        self._chk(lib().fresnel_accumulate_intensity(self._h, self._wf(wf), wp, self._map(image)), "fresnel_accumulate_intensity")
 
     def memcpy_h2d(self, dst, src_host) -> None:
         nbytes = src_host.numel() * src_host.element_size()

@@ -564,4 +564,18 @@ fresnel_status fresnel_propagate_direct(fresnel_plan *p, void *wf, double *pixel
     return FRESNEL_OK;
 }
 
+// ---- broadband image: incoherent sum over the batch ---------------------------------------------------------
+fresnel_status fresnel_accumulate_intensity(fresnel_plan *p, const void *wf, const double *weight, void *image)
+{
+    if (!p || !wf || !weight || !image) return FRESNEL_ERR_INVALID_ARG;
+    for (int b = 0; b < p->batch; ++b)
+        if (!std::isfinite(weight[b])) return FRESNEL_ERR_INVALID_ARG;
+    cudaError_t e;
+    if (p->dtype == FRESNEL_C128)
+        e = launch_intensity<double>((const double2 *)wf, (double *)image, weight, p->N, p->batch, p->sms, p->stream, &p->launches);
+    else
+        e = launch_intensity<float>((const float2 *)wf, (float *)image, weight, p->N, p->batch, p->sms, p->stream, &p->launches);
+    return e == cudaSuccess ? FRESNEL_OK : FRESNEL_ERR_CUDA;
+}
+
 } // extern "C"

@@ -44,4 +44,48 @@ cudaError_t launch_pointwise(typename cplx_of<T>::type *wf, const typename cplx_
     return cudaGetLastError();
 }
 
+// ---- broadband image -----------------------------------------
+//   image[j][k] += sum_b weight[b] * |wf[b][j][k]|^2
+// One streaming pass: every thread owns two adjacent pixels (16 or 32 bytes of wavefront per access), walks the
+// batch with the running sum in double, and touches the image once.  Weights ride in the kernel parameters.
+constexpr int kIntensityMaxBatch = 64;
+struct IntensityWeights { double w[kIntensityMaxBatch]; };
+
+template <typename T>
+__global__ void __launch_bounds__(256) intensity_kernel(const typename cplx_of<T>::type *__restrict__ wf, T *__restrict__ image,
+                                                        IntensityWeights wt, int nb, size_t plane /* N*N */)
+{
+    using C = typename cplx_of<T>::type;
+    const size_t stride = (size_t)gridDim.x * blockDim.x * 2;
+    for (size_t i = ((size_t)blockIdx.x * blockDim.x + threadIdx.x) * 2; i < plane; i += stride) {
+        double a0 = (double)image[i], a1 = (double)image[i + 1];
+        for (int b = 0; b < nb; ++b) {
+            const C u0 = wf[(size_t)b * plane + i], u1 = wf[(size_t)b * plane + i + 1];
+            a0 = fma(wt.w[b], (double)u0.x * (double)u0.x + (double)u0.y * (double)u0.y, a0);
+            a1 = fma(wt.w[b], (double)u1.x * (double)u1.x + (double)u1.y * (double)u1.y, a1);
+        }
+        image[i] = (T)a0;
+        image[i + 1] = (T)a1;
+    }
+}
+
+template <typename T>
+cudaError_t launch_intensity(const typename cplx_of<T>::type *wf, T *image, const double *weight, int N, int batch, int sms,
+                             cudaStream_t stream, unsigned long long *launches)
+{
+    const size_t plane = (size_t)N * N;
+    for (int b0 = 0; b0 < batch; b0 += kIntensityMaxBatch) {
+        IntensityWeights wt;
+        const int nb = batch - b0 < kIntensityMaxBatch ? batch - b0 : kIntensityMaxBatch;
+        for (int b = 0; b < nb; ++b) wt.w[b] = weight[b0 + b];
+        const size_t want = (plane / 2 + 255) / 256;
+        const int grid = (int)(want < (size_t)sms * 8 ? want : (size_t)sms * 8);
+        intensity_kernel<T><<<grid, 256, 0, stream>>>(wf + (size_t)b0 * plane, image, wt, nb, plane);
+        cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) return e;
+        ++*launches;
+    }
+    return cudaSuccess;
+}
+
 } // namespace fresnel

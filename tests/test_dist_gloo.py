@@ -42,8 +42,15 @@ def _worker(rank, world, port, q):
         seconds = 0.5 + 0.25 * rank                              # rank 1 is the slow one
         rate = sharding.whole_job_rate(units, seconds)
         mx = sharding.max_over_ranks([seconds, float(rank)])
+        # broadband image: every rank sums its own wavelengths, one all-reduce finishes the image
+        g = torch.Generator().manual_seed(5)
+        fields = torch.randn(16, 32, 32, dtype=torch.float64, generator=g)      # same on both ranks
+        weights = torch.linspace(0.5, 2.0, 16, dtype=torch.float64)
+        mine = (weights[lo:hi, None, None] * fields[lo:hi] ** 2).sum(0)
+        full = sharding.reduce_image(mine.clone())
+        img_err = float((full - (weights[:, None, None] * fields ** 2).sum(0)).abs().max())
         dist.barrier()
-        q.put((rank, lo, hi, rate, mx))
+        q.put((rank, lo, hi, rate, mx, img_err))
     finally:
         dist.destroy_process_group()
 
@@ -63,8 +70,11 @@ def test_two_rank_timing_reduction_gloo():
     for o in out:
         assert o[3] == pytest.approx(160 / 0.75)                 # all units / slowest rank
         assert o[4] == [0.75, 1.0]
+        assert o[5] <= 1e-12                                     # sharded broadband image == unsharded
 
 
 def test_single_process_is_identity():
     assert sharding.max_over_ranks([1.5, 2.0]) == [1.5, 2.0]
     assert sharding.whole_job_rate(20, 0.5) == 40
+    t = torch.ones(4, 4)
+    assert sharding.reduce_image(t) is t and bool((t == 1).all())

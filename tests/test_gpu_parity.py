@@ -187,6 +187,26 @@ def test_mask_large_opd_both_phasor_branches(torch_cuda, B, oracle, dtype):
     assert rel_batch(d.cpu().numpy(), want) <= TOL[dtype]
 
 
+@pytest.mark.parametrize("dtype,N,batch", [("c128", 256, 3), ("c64", 512, 2), ("c128", 1024, 1), ("c64", 128, 70)])
+def test_accumulate_intensity(torch_cuda, B, oracle, dtype, N, batch):
+    """Broadband image (NEXT-3): image += sum_b w_b |U_b|^2 against the oracle, on top of a
+    non-zero image, batch both below and above the 64 weights one launch carries."""
+    u = field(N, 1300 + N, batch, dtype)
+    w = np.random.Generator(np.random.PCG64(N)).uniform(0.1, 2.0, batch)
+    img0 = np.random.Generator(np.random.PCG64(N + 1)).uniform(0.0, 1.0, (N, N))
+    plan = B.Plan(N, batch, dtype)
+    d = to_dev(torch_cuda, u, dtype)
+    img = map_dev(torch_cuda, img0, dtype)
+    plan.accumulate_intensity(d, w, img)
+    want = map_host(img0, dtype).copy()
+    for b in range(batch):
+        want = oracle.accumulate_intensity(u[b], w[b], want)
+    got = img.cpu().numpy().astype(np.float64)
+    assert np.linalg.norm(got - want) / np.linalg.norm(want) <= (1e-14 if dtype == "c128" else 1e-6)
+    # the wavefront is read only
+    assert rel_batch(d.cpu().numpy(), u) <= (1e-7 if dtype == "c64" else 0.0)
+
+
 def test_config1(torch_cuda, B, oracle):
     from paper_1806_06467_b200 import inputs
     wl = inputs.config1()

@@ -92,7 +92,9 @@ col_tma_kernel(PassArgs<T> a, const __grid_constant__ CUtensorMap tmap)
     const int col0 = blockIdx.x * W;
 
     if (tid == 0) mbar_init(&full_bar, 1);
+    pdl_launch_dependents();
     __syncthreads();
+    pdl_wait();                                      // the row pass has finished: the wavefront may be read
     if (tid == 0) {
         mbar_expect_tx(&full_bar, (uint32_t)(N * ROW_BYTES));
 #pragma unroll 1
@@ -201,8 +203,7 @@ cudaError_t launch_col_tma(const PassArgs<T> &a, const CUtensorMap &tmap, int ba
         dim3 grid(N / G::W, batch, 1);
         PassArgs<T> b = a;
         if (b.prefetch_distance < 0) b.prefetch_distance = -b.prefetch_distance * G::MINB;
-        kern<<<grid, G::threads, G::smem + 1024, stream>>>(b, tmap);
-        return cudaGetLastError();
+        return launch_pdl(kern, grid, dim3(G::threads), G::smem + 1024, stream, b.pdl != 0, b, tmap);
     }
 }
 

@@ -53,6 +53,7 @@ struct fresnel_plan {
     int prefetch = 0;                   // L2 prefetch distance in tiles (see pass_kernel.cuh)
     int tma_w = 0;                      // columns per TMA tile of the column pass (0: not used for this N)
     int sms = 148;
+    int pdl = 1;                        // programmatic dependent launch of the pass kernels (FRESNEL_PDL=0: off, A/B timing)
     CUtensorMap tmap{};                  // tensor map of the wavefront last seen by the column pass
     const void *tmap_wf = nullptr;
     cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};   // profiling hook, see fresnel_plan_record_pass_events
@@ -261,7 +262,7 @@ bool make_tensor_map(fresnel_plan *p, void *wf)
 }
 
 // ---- pass launch by (dtype, N) ---------------------------------------------------------------------
-fresnel_status run_pass(fresnel_plan *p, bool col, int mode, void *wf, const void *pre, const void *mid,
+fresnel_status run_pass(fresnel_plan *p, bool col, int mode, void *wf, const void *pre, const void *rowfac, const void *mid,
                         const void *amp, const void *opd, double scale)
 {
     cudaError_t e = cudaErrorInvalidValue;
@@ -273,9 +274,9 @@ fresnel_status run_pass(fresnel_plan *p, bool col, int mode, void *wf, const voi
     const int prefetch = (!col && (wf_bytes > ((size_t)64 << 20) || amp || opd)) ? p->prefetch : 0;
     if (p->dtype == FRESNEL_C128) {
         PassArgs<double> a;
-        a.wf = (double2 *)wf; a.pre = (const double2 *)pre; a.mid = (const double2 *)mid;
+        a.wf = (double2 *)wf; a.pre = (const double2 *)pre; a.mid = (const double2 *)mid; a.rowfac = (const double2 *)rowfac;
         a.tw = (const double2 *)p->tw; a.amp = (const double *)amp; a.opd = (const double *)opd;
-        a.inv_lambda = p->scal_dev; a.scale = scale; a.prefetch_distance = prefetch;
+        a.inv_lambda = p->scal_dev; a.scale = scale; a.prefetch_distance = prefetch; a.pdl = p->pdl;
         switch (p->N) {
 #define FR_CASE(NN) case NN: e = tma ? launch_col_tma_f64_##NN(mode, a, p->tmap, p->batch, p->stream)           \
                                    : launch_pass_f64_##NN(col, mode, a, p->batch, p->stream); break;
@@ -284,9 +285,9 @@ fresnel_status run_pass(fresnel_plan *p, bool col, int mode, void *wf, const voi
         }
     } else {
         PassArgs<float> a;
-        a.wf = (float2 *)wf; a.pre = (const float2 *)pre; a.mid = (const float2 *)mid;
+        a.wf = (float2 *)wf; a.pre = (const float2 *)pre; a.mid = (const float2 *)mid; a.rowfac = (const float2 *)rowfac;
         a.tw = (const float2 *)p->tw; a.amp = (const float *)amp; a.opd = (const float *)opd;
-        a.inv_lambda = p->scal_dev; a.scale = (float)scale; a.prefetch_distance = prefetch;
+        a.inv_lambda = p->scal_dev; a.scale = (float)scale; a.prefetch_distance = prefetch; a.pdl = p->pdl;
         switch (p->N) {
 #define FR_CASE(NN) case NN: e = tma ? launch_col_tma_f32_##NN(mode, a, p->tmap, p->batch, p->stream)           \
                                    : launch_pass_f32_##NN(col, mode, a, p->batch, p->stream); break;
@@ -306,10 +307,12 @@ fresnel_status run_two_passes(fresnel_plan *p, int mode, void *wf, const void *p
     const bool ev = p->ev_armed;
     p->ev_armed = false;
     if (ev && cudaEventRecord(p->ev[0], p->stream) != cudaSuccess) return FRESNEL_ERR_CUDA;
-    fresnel_status st = run_pass(p, false, mode, wf, pre, mid, amp, opd, scale);
+    // the input chirp is separable: its x-part rides on the load of the row pass, its y-part (one factor per
+    // row) on the store of the row pass, so the column pass has no input table at all
+    fresnel_status st = run_pass(p, false, mode, wf, pre, pre, mid, amp, opd, scale);
     if (st != FRESNEL_OK) return st;
     if (ev && cudaEventRecord(p->ev[1], p->stream) != cudaSuccess) return FRESNEL_ERR_CUDA;
-    st = run_pass(p, true, mode, wf, pre, mid, nullptr, nullptr, scale);
+    st = run_pass(p, true, mode, wf, nullptr, nullptr, mid, nullptr, nullptr, scale);
     if (st != FRESNEL_OK) return st;
     if (ev && cudaEventRecord(p->ev[2], p->stream) != cudaSuccess) return FRESNEL_ERR_CUDA;
     return FRESNEL_OK;
@@ -379,6 +382,7 @@ fresnel_status fresnel_plan_create(fresnel_plan **out, int N, int batch, fresnel
         const char *pf = std::getenv("FRESNEL_PREFETCH");          // tuning only: tiles ahead, 0 = off
         p->prefetch = pf ? std::atoi(pf) : -sms;                   // negative: auto = SMs x resident CTAs per SM
     }
+    { const char *pd = std::getenv("FRESNEL_PDL"); p->pdl = pd ? std::atoi(pd) : 1; }
     p->tma_w = std::getenv("FRESNEL_NO_TMA") ? 0 : query_tma_width(N, dtype);     // env switch: A/B timing only
     fresnel_status st = upload_twiddles(p);
     if (st == FRESNEL_OK && cudaMalloc((void **)&p->scal_dev, sizeof(double) * batch) != cudaSuccess) st = FRESNEL_ERR_ALLOC;

@@ -6,7 +6,7 @@
 //  -> FFT (MODE_FWD, MODE_CONV) or inverse FFT (MODE_INV)
 //  -> [x mid[k]]                                (transfer function H1 / output chirp / 1/N / signs)
 //  -> inverse FFT                               (MODE_CONV only)
-//  -> [x scale]
+//  -> [x scale] [x rowfac[row]]               (row pass: the y-part of the input chirp, constant along a row)
 // and writes the line back in place.  Angular-spectrum propagation is MODE_CONV over rows then
 // over columns (H is separable); fft2d and direct Fresnel are MODE_FWD/MODE_INV over rows then
 // columns.  Shifts are folded into the tables ((-1)^n signs) and never touch memory.
@@ -23,13 +23,38 @@ template <typename T> struct PassArgs {
     C *wf;                    // [batch][N][N]
     const C *pre;             // [batch][N] or nullptr
     const C *mid;             // [batch][N] or nullptr
+    const C *rowfac;          // [batch][N] or nullptr (row pass only): row i of the result is multiplied by rowfac[i]
     const C *tw;              // FFT twiddle tables of this N
     const T *amp;             // [N][N] or nullptr (row pass only)
     const T *opd;             // [N][N] or nullptr (row pass only)
     const double *inv_lambda; // [batch] 1/lambda (only read when opd != nullptr)
     T scale;                  // applied last when != 1
     int prefetch_distance;    // tiles ahead to prefetch into L2 (0: off); ~ number of resident CTAs
+    int pdl;                  // launched with programmatic stream serialization
 };
+
+// Programmatic dependent launch: every pass kernel depends on ALL of the previous pass (a 2-D transform is
+// two global transposes), so kernels cannot overlap their work -- but the next kernel's launch latency and
+// prologue can hide under the previous kernel's last wave.  A pass kernel lets its dependents launch at once
+// and waits for its own predecessor right before its first global access.
+FR_DEV void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+FR_DEV void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
+template <typename... KArgs, typename... Args>
+cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t stream, bool pdl, Args... args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = stream;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = pdl ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kern, args...);
+}
 
 // bulk L2 prefetch of a contiguous range (bytes: multiple of 16)
 FR_DEV void l2_prefetch_bulk(const void *p, uint32_t bytes)
@@ -122,6 +147,8 @@ __global__ void __launch_bounds__(W *(N / 16), MINB) pass_kernel(PassArgs<T> a)
     const size_t gstride = COL ? (size_t)N : (size_t)1;
     C *g = a.wf + (size_t)b * N * N + (COL ? (size_t)idx : (size_t)idx * N);
 
+    pdl_launch_dependents();
+    pdl_wait();
     C v[16];
 #pragma unroll
     for (int r = 0; r < 16; ++r) v[r] = g[(size_t)(j + r * TL) * gstride];
@@ -173,6 +200,15 @@ __global__ void __launch_bounds__(W *(N / 16), MINB) pass_kernel(PassArgs<T> a)
     if (a.scale != (T)1) {
 #pragma unroll
         for (int r = 0; r < 16; ++r) { v[r].x *= a.scale; v[r].y *= a.scale; }
+    }
+    if constexpr (!COL) {
+        // the y-part of a separable input chirp is one factor per row: applied here, after the (linear) row
+        // transform, it saves the column pass a table load and a multiply on its critical path
+        if (a.rowfac != nullptr) {
+            const C c = ldg_c(a.rowfac + (size_t)b * N + idx);
+#pragma unroll
+            for (int r = 0; r < 16; ++r) v[r] = cmul(v[r], c);
+        }
     }
 #pragma unroll
     for (int r = 0; r < 16; ++r) g[(size_t)(j + r * TL) * gstride] = v[r];
@@ -246,8 +282,7 @@ cudaError_t launch_pass(const PassArgs<T> &a, int batch, cudaStream_t stream)
     dim3 grid(N / G::W, batch, 1);
     PassArgs<T> b = a;
     if (b.prefetch_distance < 0) b.prefetch_distance = -b.prefetch_distance * G::MINB;
-    kern<<<grid, G::threads, G::smem, stream>>>(b);
-    return cudaGetLastError();
+    return launch_pdl(kern, grid, dim3(G::threads), G::smem, stream, b.pdl != 0, b);
 }
 
 } // namespace fresnel

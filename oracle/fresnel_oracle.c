@@ -375,3 +375,43 @@ int oracle_accumulate_intensity(const double *u, int N, double w, double *image)
     }
     return ORACLE_OK;
 }
+
+/* ------------------------------------------------------------------------------------------
+ * train of surfaces with a per-surface choice of propagator (reduced).
+ * The paper's system is "add_optic(optic, distance=...)" repeated and POPPY picks
+ * plane-to-plane or single-FFT propagation from a Gaussian pilot beam (Lawrence Eq. 82-89),
+ * which the paper does not print.  Reading g13b: with method AUTO the choice is the sampling
+ * criterion of the two discrete operators -- the angular-spectrum chirp exp(-i pi lambda z f^2) is
+ * sampled without aliasing up to z_c = N dx^2 / lambda, the direct-Fresnel input chirp from z_c on --
+ * so |z| < z_c takes the angular spectrum (pixel pitch kept), |z| >= z_c the direct transform
+ * (pixel pitch becomes lambda |z| / (N dx)); z == 0 propagates nothing.
+ * One wavefront; surfaces applied literally one after the other.
+ *   f[s], z[s], method[s] (0 = angular spectrum, 1 = direct, 2 = auto); amp[s], opd[s] may be NULL.
+ *   used[s] (optional) receives 0 / 1 / -1 (no propagation).  *dx_inout is the running pixel pitch.
+ * ------------------------------------------------------------------------------------------ */
+int oracle_system_run(double *u, int N, double *dx_inout, double lambda, int nsurf, const double *f,
+                      const double *const *amp, const double *const *opd, const double *z,
+                      const int *method, int *used)
+{
+    if (!u || !dx_inout || !f || !z || !method || nsurf < 0) return ORACLE_ERR_INVALID_ARG;
+    int rc;
+    for (int s = 0; s < nsurf; ++s) {
+        const double dx = *dx_inout;
+        if (isnan(f[s]) || f[s] == 0.0 || !isfinite(z[s])) return ORACLE_ERR_INVALID_ARG;
+        if (isfinite(f[s]) && (rc = oracle_apply_qpf(u, N, dx, lambda, -f[s])) != ORACLE_OK) return rc;
+        const double *a = amp ? amp[s] : NULL, *o = opd ? opd[s] : NULL;
+        if ((a || o) && (rc = oracle_apply_mask(u, N, a, o, lambda)) != ORACLE_OK) return rc;
+        int m = method[s];
+        if (m < 0 || m > 2) return ORACLE_ERR_INVALID_ARG;
+        if (z[s] == 0.0) { if (used) used[s] = -1; continue; }
+        if (m == 2) {
+            const long double zc = (long double)N * (long double)dx * (long double)dx / (long double)lambda;
+            m = (fabsl((long double)z[s]) < zc) ? 0 : 1;
+        }
+        if (m == 0) rc = oracle_propagate_as(u, N, dx, lambda, z[s]);
+        else        rc = oracle_propagate_direct(u, N, dx_inout, lambda, z[s]);
+        if (rc != ORACLE_OK) return rc;
+        if (used) used[s] = m;
+    }
+    return ORACLE_OK;
+}

@@ -42,6 +42,10 @@ def lib():
         L.oracle_propagate_direct.argtypes = [dp, ctypes.c_int, dp, ctypes.c_double, ctypes.c_double]
         L.oracle_surface_as.argtypes = [dp, ctypes.c_int, ctypes.c_double, ctypes.c_double, ctypes.c_double,
                                         dp, dp, ctypes.c_double]
+        pp = ctypes.POINTER(dp)
+        L.oracle_system_run.argtypes = [dp, ctypes.c_int, dp, ctypes.c_double, ctypes.c_int, dp, pp, pp, dp,
+                                        ctypes.POINTER(ctypes.c_int), ctypes.POINTER(ctypes.c_int)]
+        L.oracle_system_run.restype = ctypes.c_int
         L.oracle_accumulate_intensity.argtypes = [dp, ctypes.c_int, ctypes.c_double, dp]
         L.oracle_accumulate_intensity.restype = ctypes.c_int
         for name in ("oracle_dft2_naive", "oracle_fft2", "oracle_fftshift", "oracle_ifftshift", "oracle_fft2d",
@@ -187,3 +191,31 @@ def broadband_image(u, weights):
     for b in range(u.shape[0]):
         img = accumulate_intensity(u[b], float(np.asarray(weights)[b]), img)
     return img
+
+
+METHOD_AS, METHOD_DIRECT, METHOD_AUTO = 0, 1, 2
+
+
+def system_run(u, dx, lam, surfaces, methods=None):
+    """Train of surfaces on one wavefront (NEXT-1 reduced, reading g13b).  `surfaces`: objects
+    with .f (None/inf = no lens), .amp, .opd, .z; `methods`: per-surface 0/1/2 (default AUTO).
+    Returns (field, final pixel pitch, list of methods used: 0 AS, 1 direct, -1 none)."""
+    a, N = _prep(u)
+    n = len(surfaces)
+    dp = ctypes.POINTER(ctypes.c_double)
+    f = np.array([math.inf if s.f is None else float(s.f) for s in surfaces], dtype=np.float64)
+    z = np.array([float(s.z) for s in surfaces], dtype=np.float64)
+    m = np.array([METHOD_AUTO] * n if methods is None else list(methods), dtype=np.int32)
+    keep, amp_p, opd_p = [], (dp * max(n, 1))(), (dp * max(n, 1))()
+    for i, s in enumerate(surfaces):
+        ka, pa = _real(s.amp, N)
+        ko, po = _real(s.opd, N)
+        keep += [ka, ko]
+        amp_p[i] = pa if pa is not None else ctypes.cast(None, dp)
+        opd_p[i] = po if po is not None else ctypes.cast(None, dp)
+    dxv = ctypes.c_double(float(dx))
+    used = np.zeros(max(n, 1), dtype=np.int32)
+    _check(lib().oracle_system_run(_dptr(a), N, ctypes.byref(dxv), float(lam), n, f.ctypes.data_as(dp), amp_p, opd_p,
+                                   z.ctypes.data_as(dp), m.ctypes.data_as(ctypes.POINTER(ctypes.c_int)),
+                                   used.ctypes.data_as(ctypes.POINTER(ctypes.c_int))), "system_run")
+    return a, dxv.value, [int(x) for x in used[:n]]

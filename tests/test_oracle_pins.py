@@ -410,3 +410,53 @@ def test_p14_broadband_energy_and_gaussian_beam_intensity(oracle):
         want += wt * (w0 / wz) ** 2 * np.exp(-2 * r2 / wz ** 2)
     assert rel(img, want) <= 1e-9
     assert abs(img.sum() / (wts.sum() * (np.abs(u0) ** 2).sum()) - 1) <= 1e-13
+
+
+# ---- P15: train of surfaces with the sampling rule for the propagator (NEXT-1 reduced, reading g13b) ----
+def test_p15_system_run_auto_rule_and_closed_form(oracle):
+    from paper_1806_06467_b200 import inputs
+    wl = inputs.config2()
+    N, dx, lam, w0 = wl.N, float(wl.dx[0]), float(wl.lam[0]), 2e-3
+    # config 2: z_c = N dx^2/lam = 0.385, 0.650, 0.866 m along the chain and z = 0.5, 0.75, 1.0 -> direct every time;
+    # the result is the ABCD closed form of the three-lens chain (P5) on the final grid
+    u, d, used = oracle.system_run(wl.field[0], dx, lam, wl.surfaces)
+    assert used == [1, 1, 1]
+    q, A = abcd_chain(lam, w0, [(s.f, s.z) for s in wl.surfaces])[-1]
+    assert d == pytest.approx(3.464e-5, rel=2e-4)
+    x, y = coords(N, d)
+    assert rel(u, A * np.exp(1j * np.pi * (x * x + y * y) / (lam * q))) <= 1e-8
+    # forced angular spectrum == the surface_as chain, bit for bit; pixel pitch unchanged
+    v, dv, used = oracle.system_run(wl.field[0], dx, lam, wl.surfaces, methods=[0, 0, 0])
+    w = wl.field[0]
+    for s in wl.surfaces:
+        w = oracle.surface_as(w, dx, lam, s.f, None, None, s.z)
+    assert used == [0, 0, 0] and dv == dx and np.array_equal(v, w)
+
+
+def test_p15_system_run_threshold_masks_and_zero_distance(oracle):
+    from paper_1806_06467_b200.inputs import Surface
+    N, dx, lam = 128, 2e-5, 1e-6
+    zc = N * dx * dx / lam                                            # 0.0512 m
+    r = np.random.Generator(np.random.PCG64(31))
+    amp, opd = (r.random((N, N)) < 0.8).astype(float), r.normal(0, 15e-9, (N, N))
+    u0 = rnd(N, 32)
+    surfs = [Surface(0.3, 0.5 * zc, amp, opd), Surface(math.inf, 0.0, None, opd), Surface(-0.7, 1.5 * zc), Surface(math.inf, -0.25 * zc)]
+    u, d, used = oracle.system_run(u0, dx, lam, surfs)
+    assert used[:3] == [0, -1, 1]                                     # below z_c: AS; z = 0: none; above: direct
+    d2 = lam * 1.5 * zc / (N * dx)
+    assert d == pytest.approx(d2, rel=1e-15)
+    assert used[3] == 0                                               # new pitch 1.5 dx -> z_c grows to 2.25 z_c
+    # the literal composition
+    w = oracle.propagate_as(oracle.apply_mask(oracle.apply_qpf(u0, dx, lam, -0.3), amp, opd, lam), dx, lam, 0.5 * zc)
+    w = oracle.apply_mask(w, None, opd, lam)
+    w, dw = oracle.propagate_direct(oracle.apply_qpf(w, dx, lam, 0.7), dx, lam, 1.5 * zc)
+    w = oracle.propagate_as(w, dw, lam, -0.25 * zc)
+    assert np.array_equal(u, w)
+    # from z_c on the rule takes the direct transform, and at z_c the two operators coincide (P9)
+    zc1 = zc * (1 + 1e-12)
+    a, da, ua = oracle.system_run(u0, dx, lam, [Surface(math.inf, zc1)])
+    b, db, ub = oracle.system_run(u0, dx, lam, [Surface(math.inf, zc1)], methods=[0])
+    assert ua == [1] and ub == [0] and da == pytest.approx(dx, rel=1e-11) and rel(a, b) <= 1e-9
+    assert oracle.system_run(u0, dx, lam, [Surface(math.inf, zc * (1 - 1e-12))])[2] == [0]
+    with pytest.raises(oracle.OracleError):
+        oracle.system_run(u0, dx, lam, [Surface(0.0, 0.1)])

@@ -123,6 +123,33 @@ fresnel_status fresnel_propagate_direct(fresnel_plan *p, void *wf, double *pixel
 fresnel_status fresnel_surface_as(fresnel_plan *p, void *wf, const double *pixel, const double *lambda,
                                   double f, const void *amp, const void *opd, double z);
 
+/* A train of surfaces in one call (add_optic(optic, distance=...) repeated; SURVEY.md
+ * sec. 8(f) NEXT-1, reduced).  Surface s = thin lens f (+-INFINITY: none), optic phasor (amp, opd; NULL: none),
+ * then propagation by z with `method`:
+ *     FRESNEL_METHOD_AS      angular spectrum (fresnel_surface_as): pixel pitch kept;
+ *     FRESNEL_METHOD_DIRECT  direct Fresnel: pixel pitch becomes lambda*|z|/(N*dx); the lens chirp is merged
+ *                            into the propagator's input chirp and the phasor rides on the row pass, so the
+ *                            surface still costs two passes;
+ *     FRESNEL_METHOD_AUTO    POPPY chooses from a Gaussian pilot beam (Lawrence Eq. 82-89), which the
+ *                            paper does not print; reading g13b takes the sampling criterion of the two discrete
+ *                            operators instead: |z| < z_c = N*dx^2/lambda -> angular spectrum, else direct.
+ *                            Every batch element must fall on the same side of its own z_c, otherwise
+ *                            FRESNEL_ERR_UNSUPPORTED (split the batch or force a method).
+ * z == 0 applies the optic only.  pixel_inout (HOST, length batch) carries the running pixel pitch and holds the
+ * final one on return; method_used (HOST, length nsurf, may be NULL) receives 0 / 1, or -1 where z == 0.
+ * All surfaces are validated before anything is enqueued; the calls enqueue only, so a train can be captured
+ * into one CUDA graph. */
+typedef struct {
+    double f;
+    const void *amp;
+    const void *opd;
+    double z;
+    int method;
+} fresnel_surface;
+enum { FRESNEL_METHOD_AS = 0, FRESNEL_METHOD_DIRECT = 1, FRESNEL_METHOD_AUTO = 2 };
+fresnel_status fresnel_system_run(fresnel_plan *p, void *wf, double *pixel_inout, const double *lambda,
+                                  const fresnel_surface *surf, int nsurf, int *method_used);
+
 /* Broadband (polychromatic) image: the incoherent, weighted sum of the batch's monochromatic intensities
  * ("calculations must be repeated for all of the wavelengths"; one process per wavelength in
  * the paper):

@@ -28,11 +28,18 @@ C64, C128 = 0, 1
 SYMBOLS = (
     "fresnel_plan_create", "fresnel_plan_set_stream", "fresnel_plan_synchronize", "fresnel_plan_destroy",
     "fresnel_plan_launch_count", "fresnel_plan_record_pass_events", "fresnel_apply_qpf", "fresnel_apply_mask", "fresnel_fft2d",
-    "fresnel_propagate_as", "fresnel_propagate_direct", "fresnel_surface_as", "fresnel_accumulate_intensity", "fresnel_memcpy_h2d",
+    "fresnel_propagate_as", "fresnel_propagate_direct", "fresnel_surface_as", "fresnel_system_run", "fresnel_accumulate_intensity", "fresnel_memcpy_h2d",
     "fresnel_memcpy_d2h", "fresnel_status_string", "fresnel_version",
 )
 
 _lib = None
+
+METHOD_AS, METHOD_DIRECT, METHOD_AUTO = 0, 1, 2
+
+
+class _Surface(ctypes.Structure):       # fresnel_surface of include/fresnel.h
+    _fields_ = [("f", ctypes.c_double), ("amp", ctypes.c_void_p), ("opd", ctypes.c_void_p),
+                ("z", ctypes.c_double), ("method", ctypes.c_int)]
 
 
 class FresnelError(RuntimeError):
@@ -64,6 +71,7 @@ def lib() -> ctypes.CDLL:
     L.fresnel_propagate_as.argtypes = [vp, vp, dp, dp, cd]
     L.fresnel_propagate_direct.argtypes = [vp, vp, dp, dp, cd]
     L.fresnel_surface_as.argtypes = [vp, vp, dp, dp, cd, vp, vp, cd]
+    L.fresnel_system_run.argtypes = [vp, vp, dp, dp, ctypes.POINTER(_Surface), ci, ctypes.POINTER(ci)]
     L.fresnel_accumulate_intensity.argtypes = [vp, vp, dp, vp]
     L.fresnel_memcpy_h2d.argtypes = [vp, vp, vp, ctypes.c_size_t]
     L.fresnel_memcpy_d2h.argtypes = [vp, vp, vp, ctypes.c_size_t]
@@ -193,6 +201,27 @@ class Plan:
         ff = math.inf if f is None else float(f)
         self._chk(lib().fresnel_surface_as(self._h, self._wf(wf), pp, lp, ff, self._map(amp), self._map(opd), float(z)),
                   "fresnel_surface_as")
+
+    def system_run(self, wf, pixel, lam, surfaces, maps=None, methods=None):
+        """Train of surfaces in one call.  surfaces: objects with .f, .z; maps[i] = (amp, opd) device tensors or
+        None; methods: per-surface METHOD_AS / METHOD_DIRECT / METHOD_AUTO (default AUTO).
+        Returns (final pixel pitch per batch element, methods used)."""
+        n = len(surfaces)
+        arr = (_Surface * max(n, 1))()
+        for i, s in enumerate(surfaces):
+            amp, opd = (maps[i] if maps is not None else (None, None))
+            arr[i].f = math.inf if s.f is None else float(s.f)
+            arr[i].amp = self._map(amp).value
+            arr[i].opd = self._map(opd).value
+            arr[i].z = float(s.z)
+            arr[i].method = METHOD_AUTO if methods is None else int(methods[i])
+        pa, _ = _darr(pixel, self.batch)
+        pa = pa.copy()
+        pp = pa.ctypes.data_as(ctypes.POINTER(ctypes.c_double))
+        _, lp = _darr(lam, self.batch)
+        used = (ctypes.c_int * max(n, 1))()
+        self._chk(lib().fresnel_system_run(self._h, self._wf(wf), pp, lp, arr, n, used), "fresnel_system_run")
+        return pa, [int(used[i]) for i in range(n)]
 
     def accumulate_intensity(self, wf, weight, image) -> None:
         """image += sum_b weight[b] * |wf[b]|^2 (image: real N x N device tensor of the plan's precision)."""

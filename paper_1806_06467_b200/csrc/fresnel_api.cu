@@ -540,31 +540,97 @@ fresnel_status fresnel_propagate_as(fresnel_plan *p, void *wf, const double *pix
 }
 
 // ---- direct (single-FFT) Fresnel ---------------------------------------------------------------------
-fresnel_status fresnel_propagate_direct(fresnel_plan *p, void *wf, double *pixel_inout, const double *lambda, double z)
+} // extern "C"
+
+namespace {
+
+// [thin lens f] -> [optic phasor] -> direct Fresnel propagation by z, in the two passes of the transform:
+// the lens chirp and the input chirp of the propagator are the same kind of factor, so their
+// coefficients are added (long double) and ONE table serves both; the optic phasor rides on the row-pass load.
+fresnel_status direct_impl(fresnel_plan *p, void *wf, double *pixel_inout, const double *lambda, double z,
+                           double f, const void *amp, const void *opd)
 {
-    if (!p || !wf || !valid_positive(pixel_inout, p ? p->batch : 0) || !valid_positive(lambda, p->batch)) return FRESNEL_ERR_INVALID_ARG;
-    if (!std::isfinite(z) || z == 0.0) return FRESNEL_ERR_INVALID_ARG;
     ++p->call_id;
     const bool force = capturing(p);
+    const bool lens = std::isfinite(f);
     std::vector<ChirpSpec> kin(p->batch), kout(p->batch);
     std::vector<double> dx_out(p->batch);
     for (int b = 0; b < p->batch; ++b) {
         const double dx = pixel_inout[b];
         const long double dxo = (long double)lambda[b] * fabsl((long double)z) / ((long double)p->N * (long double)dx);
         dx_out[b] = (double)dxo;
-        kin[b] = make_spec(qpf_coeff(dx, lambda[b], z), 1.0, 0.0);
+        long double cin = qpf_coeff(dx, lambda[b], z);
+        if (lens) cin += qpf_coeff(dx, lambda[b], -(long double)f);
+        kin[b] = make_spec(cin, 1.0, 0.0);
         // per-axis share of dx^2/(i lambda z): dx/sqrt(lambda |z|) * exp(-+ i pi/4)
         const double a1 = (double)((long double)dx / sqrtl((long double)lambda[b] * fabsl((long double)z)));
         kout[b] = make_spec(qpf_coeff(dx_out[b], lambda[b], z), a1, z > 0 ? -0.125 : 0.125);
     }
     // the (-1)^n of the centred transform rides on both tables
     TableRequest r[2] = {request_table(p, 0, 1, kin, force), request_table(p, 0, 1, kout, force)};
-    fresnel_status st = flush_builds(p, r, 2, nullptr);
+    std::vector<double> tmp;
+    const double *scal = opd ? need_inv_lambda(p, lambda, tmp, force) : nullptr;
+    fresnel_status st = flush_builds(p, r, 2, scal);
     if (st != FRESNEL_OK) return st;
     const int mode = z > 0 ? MODE_FWD : MODE_INV;
-    st = run_two_passes(p, mode, wf, p->slots[r[0].slot].dev, p->slots[r[1].slot].dev, nullptr, nullptr, 1.0);
+    st = run_two_passes(p, mode, wf, p->slots[r[0].slot].dev, p->slots[r[1].slot].dev, amp, opd, 1.0);
     if (st != FRESNEL_OK) return st;
     for (int b = 0; b < p->batch; ++b) pixel_inout[b] = dx_out[b];
+    return FRESNEL_OK;
+}
+
+} // namespace
+
+extern "C" {
+
+fresnel_status fresnel_propagate_direct(fresnel_plan *p, void *wf, double *pixel_inout, const double *lambda, double z)
+{
+    if (!p || !wf || !valid_positive(pixel_inout, p ? p->batch : 0) || !valid_positive(lambda, p->batch)) return FRESNEL_ERR_INVALID_ARG;
+    if (!std::isfinite(z) || z == 0.0) return FRESNEL_ERR_INVALID_ARG;
+    return direct_impl(p, wf, pixel_inout, lambda, z, INFINITY, nullptr, nullptr);
+}
+
+// ---- train of surfaces ---------------------------------------------------------------------------------
+fresnel_status fresnel_system_run(fresnel_plan *p, void *wf, double *pixel_inout, const double *lambda,
+                                  const fresnel_surface *surf, int nsurf, int *method_used)
+{
+    if (!p || !wf || nsurf < 0 || (nsurf > 0 && !surf)) return FRESNEL_ERR_INVALID_ARG;
+    if (!valid_positive(pixel_inout, p->batch) || !valid_positive(lambda, p->batch)) return FRESNEL_ERR_INVALID_ARG;
+    // dry run on the host: validate everything and fix the propagator of every surface before anything is enqueued
+    std::vector<int> method(nsurf);
+    std::vector<long double> dx(p->batch);
+    for (int b = 0; b < p->batch; ++b) dx[b] = pixel_inout[b];
+    for (int s = 0; s < nsurf; ++s) {
+        const fresnel_surface &q = surf[s];
+        if (std::isnan(q.f) || q.f == 0.0 || !std::isfinite(q.z)) return FRESNEL_ERR_INVALID_ARG;
+        if (q.method != FRESNEL_METHOD_AS && q.method != FRESNEL_METHOD_DIRECT && q.method != FRESNEL_METHOD_AUTO) return FRESNEL_ERR_INVALID_ARG;
+        if (q.z == 0.0) { method[s] = -1; continue; }
+        int m = q.method;
+        if (m == FRESNEL_METHOD_AUTO) {
+            int n_as = 0;
+            for (int b = 0; b < p->batch; ++b) {
+                const long double zc = (long double)p->N * dx[b] * dx[b] / (long double)lambda[b];
+                if (fabsl((long double)q.z) < zc) ++n_as;
+            }
+            if (n_as == p->batch) m = FRESNEL_METHOD_AS;
+            else if (n_as == 0) m = FRESNEL_METHOD_DIRECT;
+            else return FRESNEL_ERR_UNSUPPORTED;        // the batch straddles z_c: split it or force a method
+        }
+        method[s] = m;
+        if (m == FRESNEL_METHOD_DIRECT)
+            for (int b = 0; b < p->batch; ++b) {
+                dx[b] = (long double)(double)((long double)lambda[b] * fabsl((long double)q.z) / ((long double)p->N * (long double)(double)dx[b]));
+                if (!(dx[b] > 0.0L) || !std::isfinite((double)dx[b])) return FRESNEL_ERR_INVALID_ARG;
+            }
+    }
+    for (int s = 0; s < nsurf; ++s) {
+        const fresnel_surface &q = surf[s];
+        fresnel_status st;
+        if (method[s] == FRESNEL_METHOD_DIRECT) st = direct_impl(p, wf, pixel_inout, lambda, q.z, q.f, q.amp, q.opd);
+        else st = fresnel_surface_as(p, wf, pixel_inout, lambda, q.f, q.amp, q.opd, q.z);   // z == 0: optic only
+        if (st != FRESNEL_OK) return st;
+        if (method_used) method_used[s] = method[s];
+    }
     return FRESNEL_OK;
 }
 

@@ -338,3 +338,94 @@ def test_cuda_graph_capture_of_a_chain(torch_cuda, B, oracle):
     for surf in wl.surfaces:
         o = oracle.surface_as(o, wl.dx[0], wl.lam[0], surf.f, None, None, surf.z)
     assert rel_batch(d.cpu().numpy(), o[None]) <= 1e-11
+
+
+# ---- train of surfaces (NEXT-1 reduced, reading g13b) ---------------------------------------------
+def test_system_run_config2_auto_takes_direct_and_matches_oracle(torch_cuda, B, oracle):
+    from paper_1806_06467_b200 import inputs
+    wl = inputs.config2()
+    plan = B.Plan(wl.N, 1, "c128")
+    d = to_dev(torch_cuda, wl.field, "c128")
+    px, used = plan.system_run(d, wl.dx, wl.lam, wl.surfaces)
+    want, dxo, used_o = oracle.system_run(wl.field[0], wl.dx[0], wl.lam[0], wl.surfaces)
+    assert used == used_o == [1, 1, 1]
+    assert px[0] == pytest.approx(dxo, rel=1e-15)
+    assert rel_batch(d.cpu().numpy(), want[None]) <= 1e-11
+    # forced angular spectrum: the surface_as chain
+    d = to_dev(torch_cuda, wl.field, "c128")
+    px, used = plan.system_run(d, wl.dx, wl.lam, wl.surfaces, methods=[B.METHOD_AS] * 3)
+    want, _, _ = oracle.system_run(wl.field[0], wl.dx[0], wl.lam[0], wl.surfaces, methods=[0, 0, 0])
+    assert used == [0, 0, 0] and px[0] == wl.dx[0]
+    assert rel_batch(d.cpu().numpy(), want[None]) <= 1e-11
+
+
+@pytest.mark.parametrize("dtype", ["c128", "c64"])
+def test_system_run_mixed_train_with_masks_and_batch(torch_cuda, B, oracle, dtype):
+    """Lens + maps + AS below z_c, optic only at z = 0, lens merged into the direct transform above z_c (also
+    with a mask on that surface and with z < 0), two wavelengths on the same side of their z_c."""
+    from paper_1806_06467_b200 import inputs
+    from paper_1806_06467_b200.inputs import Surface
+    N = 512
+    dx, lam = np.array([2e-5, 2e-5]), np.array([1.0e-6, 0.9e-6])
+    zc = N * dx[0] ** 2 / lam[0]                                    # 0.2048 m (0.2276 m for the second wavelength)
+    amp = inputs.circular_aperture(N, N / 3)
+    opd = inputs.psd_map(N, 2e-5, 3.0, 15e-9, 41)
+    surfs = [Surface(0.6, 0.4 * zc, amp, opd), Surface(math.inf, 0.0, None, opd), Surface(-0.9, 1.7 * zc, amp, opd),
+             Surface(0.8, -1.3 * 1.7 ** 2 * zc), Surface(math.inf, 0.3 * zc)]
+    u = field(N, 77, 2, dtype)
+    plan = B.Plan(N, 2, dtype)
+    maps = [(map_dev(torch_cuda, s.amp, dtype), map_dev(torch_cuda, s.opd, dtype)) for s in surfs]
+    d = to_dev(torch_cuda, u, dtype)
+    px, used = plan.system_run(d, dx, lam, surfs, maps=maps)
+    assert used == [0, -1, 1, 1, 0]
+    got = d.cpu().numpy().reshape(2, N, N)
+    for b in range(2):
+        hs = [Surface(s.f, s.z, map_host(s.amp, dtype), map_host(s.opd, dtype)) for s in surfs]
+        want, dxo, used_o = oracle.system_run(u[b], dx[b], lam[b], hs)
+        assert used_o == used
+        assert px[b] == pytest.approx(dxo, rel=1e-14)
+        assert rel_batch(got[b][None], want[None]) <= TOL[dtype]
+
+
+def test_system_run_errors_enqueue_nothing(torch_cuda, B):
+    from paper_1806_06467_b200.inputs import Surface
+    N = 256
+    plan = B.Plan(N, 2, "c128")
+    u = field(N, 5, 2)
+    d = to_dev(torch_cuda, u, "c128")
+    l0 = plan.launch_count()
+    dx, lam = np.array([1e-5, 1e-5]), np.array([0.5e-6, 1.0e-6])     # z_c = 0.0512 and 0.0256 m
+    with pytest.raises(B.FresnelError) as e:                         # the batch straddles z_c
+        plan.system_run(d, dx, lam, [Surface(math.inf, 0.01), Surface(math.inf, 0.04)])
+    assert e.value.status == 2
+    with pytest.raises(B.FresnelError) as e:                         # bad focal length in the LAST surface
+        plan.system_run(d, dx, lam, [Surface(math.inf, 0.01), Surface(0.0, 0.01)])
+    assert e.value.status == 1
+    assert plan.launch_count() == l0                                 # validated before anything was enqueued
+    assert rel_batch(d.cpu().numpy(), u) == 0.0
+    # forcing the method resolves the straddle
+    plan.system_run(d, dx, lam, [Surface(math.inf, 0.04)], methods=[B.METHOD_AS])
+
+
+def test_system_run_as_one_cuda_graph(torch_cuda, B, oracle):
+    torch = torch_cuda
+    from paper_1806_06467_b200 import inputs
+    wl = inputs.config2()
+    s = torch.cuda.Stream()
+    plan = B.Plan(wl.N, 1, "c128", stream=s)
+    d = to_dev(torch, wl.field, "c128")
+    src = d.clone()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(s):
+        plan.system_run(d, wl.dx, wl.lam, wl.surfaces)              # warm-up outside capture
+        s.synchronize()
+        d.copy_(src)
+        s.synchronize()
+        with torch.cuda.graph(g, stream=s):
+            plan.system_run(d, wl.dx, wl.lam, wl.surfaces)
+    d.copy_(src)
+    torch.cuda.synchronize()
+    g.replay()
+    torch.cuda.synchronize()
+    want, _, _ = oracle.system_run(wl.field[0], wl.dx[0], wl.lam[0], wl.surfaces)
+    assert rel_batch(d.cpu().numpy(), want[None]) <= 1e-11

@@ -209,6 +209,7 @@ int main(){
     run_insm<float, 2048, 4, 0>("transform pair", hz); run_insm<float, 2048, 8, 0>("transform pair", hz);
     run_insm<float, 2048, 8, 0, 32>("pair, warp-local sync", hz);
     run_insm<float, 4096, 4, 1>("butterflies", hz); run_insm<float, 4096, 4, 2>("exchanges", hz); run_insm<float, 4096, 4, 0>("transform pair", hz);
+    run_insm<double, 8192, 1, 0>("transform pair", hz); run_insm<float, 8192, 2, 0>("transform pair", hz);
     run_overlap<8, 0, 16>(hz); run_overlap<0, 8, 16>(hz); run_overlap<8, 8, 16>(hz); run_overlap<8, 8, 4>(hz);
   }
   return 0;

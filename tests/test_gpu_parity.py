@@ -254,6 +254,54 @@ def test_config3_reduced_chain(torch_cuda, B, oracle):
             assert rel_batch(d.cpu().numpy(), o[None]) <= 1e-11, f"surface {i}"
 
 
+def test_config3_full_size_bench_step(torch_cuda, B, oracle):
+    """The step bench.py times: config 3 at its full size (N=2048, complex128, 20 surfaces with their maps), same
+    call sequence, whole field against the oracle at the end of the chain and at three surfaces on the way."""
+    from paper_1806_06467_b200 import inputs
+    wl = inputs.config3()
+    assert wl.N == 2048 and len(wl.surfaces) == 20
+    plan = B.Plan(wl.N, 1, "c128")
+    d = to_dev(torch_cuda, wl.field, "c128")
+    maps = [(map_dev(torch_cuda, s.amp, "c128"), map_dev(torch_cuda, s.opd, "c128")) for s in wl.surfaces]
+    o = wl.field[0]
+    for i, s in enumerate(wl.surfaces):
+        plan.surface_as(d, wl.dx, wl.lam, s.f, maps[i][0], maps[i][1], s.z)
+        o = oracle.surface_as(o, wl.dx[0], wl.lam[0], s.f, s.amp, s.opd, s.z)
+        if i in (0, 6, 12, 19):
+            assert rel_batch(d.cpu().numpy(), o[None]) <= 1e-11, f"surface {i}"
+
+
+def test_config5_full_size_sampled(torch_cuda, B, oracle):
+    """Config 5 at full size (16 wavelengths x 4096^2 complex64, 10 planes, one call per plane for the whole
+    batch): the first and the last wavelength against the oracle over the first 3 planes, and for ALL wavelengths
+    and all 10 planes the invariant the chain has -- lenses and propagation are unitary, so the energy after the
+    pupil mask of plane 0 is conserved."""
+    torch = torch_cuda
+    from paper_1806_06467_b200 import inputs
+    wl = inputs.config5()
+    assert wl.N == 4096 and wl.batch == 16 and len(wl.surfaces) == 10
+    plan = B.Plan(wl.N, wl.batch, "c64")
+    d = to_dev(torch, wl.field, "c64")
+    maps = [(map_dev(torch, s.amp, "c64"), map_dev(torch, s.opd, "c64")) for s in wl.surfaces]
+    picks = (0, 15)
+    o = {b: wl.field[b].astype(np.complex64).astype(np.complex128) for b in picks}
+    e_after_pupil = None
+    for i, s in enumerate(wl.surfaces):
+        plan.surface_as(d, wl.dx, wl.lam, s.f, maps[i][0], maps[i][1], s.z)
+        if i == 0:
+            e_after_pupil = (d.abs().double() ** 2).sum(dim=(-2, -1)).cpu().numpy()
+        if i < 3:
+            for b in picks:
+                o[b] = oracle.surface_as(o[b], wl.dx[b], wl.lam[b], s.f, map_host(s.amp, "c64"), map_host(s.opd, "c64"), s.z)
+            if i == 2:
+                got = d.cpu().numpy().reshape(wl.batch, wl.N, wl.N)
+                for b in picks:
+                    assert rel_batch(got[b][None], o[b][None]) <= 2e-5, f"wavelength {b}"
+                del got
+    e_end = (d.abs().double() ** 2).sum(dim=(-2, -1)).cpu().numpy()
+    assert np.all(np.abs(e_end / e_after_pupil - 1) <= 2e-5)
+
+
 def test_config5_reduced_batch(torch_cuda, B, oracle):
     """Polychromatic batch at N=512, 4 wavelengths, 10 planes, c64."""
     from paper_1806_06467_b200 import inputs

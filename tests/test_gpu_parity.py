@@ -328,6 +328,26 @@ def test_large_grids_sampled(torch_cuda, B, oracle, dtype, N):
     assert rel_batch(d.cpu().numpy(), want) <= TOL[dtype]
 
 
+@pytest.mark.parametrize("dtype,N", [("c128", 4096), ("c64", 8192)])
+def test_large_grids_fused_surface_and_direct(torch_cuda, B, oracle, dtype, N):
+    """Large grids through the fused surface (lens + amplitude + OPD + AS: phasor and chirps on the row pass,
+    per-row factor on its store) and through direct Fresnel with z < 0, whole field against the oracle."""
+    from paper_1806_06467_b200 import inputs
+    u = field(N, 2000 + N, 1, dtype)
+    dx, lam = np.array([1e-5]), np.array([633e-9])
+    amp = inputs.circular_aperture(N, N / 3)
+    opd = inputs.psd_map(N, 1e-5, 2.5, 15e-9, 2001)
+    plan = B.Plan(N, 1, dtype)
+    d = to_dev(torch_cuda, u, dtype)
+    plan.surface_as(d, dx, lam, 1.3, map_dev(torch_cuda, amp, dtype), map_dev(torch_cuda, opd, dtype), 0.2)
+    want = oracle.surface_as(u[0], dx[0], lam[0], 1.3, map_host(amp, dtype), map_host(opd, dtype), 0.2)
+    assert rel_batch(d.cpu().numpy(), want[None]) <= TOL[dtype]
+    px = plan.propagate_direct(d, dx, lam, -0.9)
+    want, dxo = oracle.propagate_direct(want, dx[0], lam[0], -0.9)
+    assert px[0] == pytest.approx(dxo, rel=1e-15)
+    assert rel_batch(d.cpu().numpy(), want[None]) <= TOL[dtype]
+
+
 def test_error_codes(torch_cuda, B):
     import ctypes
     L = B.lib()

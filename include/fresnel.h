@@ -119,7 +119,7 @@ fresnel_status fresnel_propagate_direct(fresnel_plan *p, void *wf, double *pixel
 /* One whole surface, fused ("add_optic(optic, distance=...)"):
  *     apply_qpf(z = -f)  [skipped if f is +-INFINITY]  ->  apply_mask(amp, opd)  ->  propagate_as(z)
  * in the same two passes as fresnel_propagate_as: the optic phasor and the x-chirp of the lens ride on
- * the load of the row pass, the y-chirp on the load of the column pass.  z == 0: optic only. */
+ * the load of the row pass, the y-chirp (one factor per row) on its store.  z == 0: optic only. */
 fresnel_status fresnel_surface_as(fresnel_plan *p, void *wf, const double *pixel, const double *lambda,
                                   double f, const void *amp, const void *opd, double z);
 

@@ -529,8 +529,8 @@ fresnel_status fresnel_surface_as(fresnel_plan *p, void *wf, const double *pixel
     const void *tl = lens ? p->slots[r[i_lens].slot].dev : nullptr;
     if (!prop) return run_pointwise(p, wf, tl, amp, opd);          // optic only
     const void *th = p->slots[r[i_h].slot].dev;
-    // row pass: optic phasor and x-chirp of the lens on load, FFT, x H1, inverse FFT;
-    // column pass: y-chirp of the lens on load, FFT, x H1, inverse FFT
+    // row pass: optic phasor and x-chirp of the lens on load, FFT, x H1, inverse FFT, y-chirp of the lens (one
+    // factor per row) on store;  column pass: FFT, x H1, inverse FFT
     return run_two_passes(p, MODE_CONV, wf, tl, th, amp, opd, 1.0);
 }
 

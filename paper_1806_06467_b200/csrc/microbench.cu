@@ -4,7 +4,8 @@
 //   MEASURED_PEAKS.json does not carry; and the IN-SM rates of the transform itself (no HBM): the stage code
 //   of fft_core.cuh on registers + shared memory only -- butterflies alone, exchanges alone, both -- in SM
 //   cycles per element, next to a synthetic stream that interleaves DFMA with 128-bit shared-memory traffic
-//   in every warp (what the two pipes can do when nothing orders them).   Build + run:
+//   in every warp (what the two pipes can do when nothing orders them), and warp shuffles mixed with shared-memory
+//   traffic (they share one pipe).   Build + run:
 //     python -m paper_1806_06467_b200.build --microbench && ./paper_1806_06467_b200/microbench
 #include <cstdio>
 #include <cstdlib>
@@ -175,6 +176,46 @@ template <int NM, int NX, int WARPS> void run_overlap(double clock_hz){
   cudaFree(out);
 }
 
+// do warp shuffles have a data path of their own?  NS shfl.sync (32-bit) and/or NX (STS.128 + LDS.128) pairs per warp-iteration
+template <int NS, int NX, int WARPS>
+__global__ void __launch_bounds__(WARPS * 32, 1) shflmix(int iters, float* out){
+  extern __shared__ double2 sm3[];
+  const int tid = threadIdx.x, lane = tid & 31;
+  float s[8];
+  #pragma unroll
+  for (int i = 0; i < 8; ++i) s[i] = tid + i;
+  double2 v[8];
+  #pragma unroll
+  for (int i = 0; i < 8; ++i) v[i] = make_double2(tid, i);
+  const unsigned base = (unsigned)__cvta_generic_to_shared(sm3 + tid);
+  for (int it = 0; it < iters; ++it) {
+    #pragma unroll
+    for (int u = 0; u < (NS / 8 > NX ? NS / 8 : NX); ++u) {
+      if (u < NX) asm volatile("st.shared.v2.f64 [%0], {%1, %2};" ::"r"(base + (u & 7) * WARPS * 32 * 16), "d"(v[u & 7].x), "d"(v[u & 7].y) : "memory");
+      if (u < NS / 8) {
+        #pragma unroll
+        for (int i = 0; i < 8; ++i) s[i] = __shfl_sync(0xffffffffu, s[i], (lane + 1 + i) & 31) + 1.0f;
+      }
+      if (u < NX) asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v[(u + 3) & 7].x), "=d"(v[(u + 3) & 7].y) : "r"(base + ((u + 5) & 7) * WARPS * 32 * 16) : "memory");
+    }
+  }
+  float r = 0;
+  #pragma unroll
+  for (int i = 0; i < 8; ++i) r += s[i] + (float)v[i].x + (float)v[i].y;
+  out[blockIdx.x * WARPS * 32 + tid] = r;
+}
+template <int NS, int NX, int WARPS> void run_shfl(double clock_hz){
+  float* out; CK(cudaMalloc(&out, 148 * 1024 * 4));
+  const int smem = WARPS * 32 * 8 * 16;
+  CK(cudaFuncSetAttribute(shflmix<NS, NX, WARPS>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+  const int iters = 4000;
+  float ms = timeit([&]{ shflmix<NS, NX, WARPS><<<148, WARPS * 32, smem>>>(iters, out); }, 3);
+  CK(cudaGetLastError());
+  printf("  shuffle warps/SM=%2d shfl=%3d lds+sts=%2d per warp-iteration: %7.1f clk   (shared-memory pipe alone %4.0f, shfl at 1 warp-instr/clk/SM %4.0f)\n",
+         WARPS, NS, NX * 2, ms * 1e-3 * clock_hz / iters, WARPS * NX * 2 * 4.0, (double)WARPS * NS);
+  cudaFree(out);
+}
+
 int main(){
   cudaDeviceProp p; CK(cudaGetDeviceProperties(&p,0)); printf("%s SMs=%d L2=%d MB clock=%d MHz\n",p.name,p.multiProcessorCount,p.l2CacheSize>>20,p.clockRate/1000);
   size_t n=(size_t)1<<30; // 1 GiB
@@ -211,6 +252,7 @@ int main(){
     run_insm<float, 4096, 4, 1>("butterflies", hz); run_insm<float, 4096, 4, 2>("exchanges", hz); run_insm<float, 4096, 4, 0>("transform pair", hz);
     run_insm<double, 8192, 1, 0>("transform pair", hz); run_insm<float, 8192, 2, 0>("transform pair", hz);
     run_overlap<8, 0, 16>(hz); run_overlap<0, 8, 16>(hz); run_overlap<8, 8, 16>(hz); run_overlap<8, 8, 4>(hz);
+    run_shfl<64, 0, 16>(hz); run_shfl<0, 8, 16>(hz); run_shfl<64, 8, 16>(hz);
   }
   return 0;
 }

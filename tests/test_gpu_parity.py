@@ -497,3 +497,21 @@ def test_system_run_as_one_cuda_graph(torch_cuda, B, oracle):
     torch.cuda.synchronize()
     want, _, _ = oracle.system_run(wl.field[0], wl.dx[0], wl.lam[0], wl.surfaces)
     assert rel_batch(d.cpu().numpy(), want[None]) <= 1e-11
+
+
+def test_table_cache_eviction_long_train(torch_cuda, B, oracle):
+    """40 surfaces with distinct lenses and distances need 80 chirp tables, more than the plan caches (64): the
+    least-recently-used slots are rebuilt in stream order.  Run the train twice (second time with a partly stale
+    cache) against the oracle."""
+    from paper_1806_06467_b200.inputs import Surface
+    N, dx, lam = 128, np.array([2e-5]), np.array([0.8e-6])
+    r = np.random.Generator(np.random.PCG64(404))
+    surfs = [Surface(float(r.uniform(0.3, 2.0)), float(r.uniform(0.002, 0.02))) for _ in range(40)]
+    u = field(N, 405, 1)
+    plan = B.Plan(N, 1, "c128")
+    want, _, _ = oracle.system_run(u[0], dx[0], lam[0], surfs, methods=[0] * 40)
+    for _ in range(2):
+        d = to_dev(torch_cuda, u, "c128")
+        px, used = plan.system_run(d, dx, lam, surfs, methods=[B.METHOD_AS] * 40)
+        assert used == [0] * 40 and px[0] == dx[0]
+        assert rel_batch(d.cpu().numpy(), want[None]) <= 1e-11

@@ -5,7 +5,8 @@
 //   of fft_core.cuh on registers + shared memory only -- butterflies alone, exchanges alone, both -- in SM
 //   cycles per element, next to a synthetic stream that interleaves DFMA with 128-bit shared-memory traffic
 //   in every warp (what the two pipes can do when nothing orders them), and warp shuffles mixed with shared-memory
-//   traffic (they share one pipe).   Build + run:
+//   traffic (they share one pipe), and register <-> tensor-memory moves (tcgen05.st/ld) beside shared-memory traffic
+//   (a separate, faster path).   Build + run:
 //     python -m paper_1806_06467_b200.build --microbench && ./paper_1806_06467_b200/microbench
 #include <cstdio>
 #include <cstdlib>
@@ -216,6 +217,67 @@ template <int NS, int NX, int WARPS> void run_shfl(double clock_hz){
   cudaFree(out);
 }
 
+// tensor memory as an exchange path: NT (tcgen05.st + tcgen05.ld, 32x32b.x16) pairs and/or NX (STS.128 + LDS.128)
+// pairs per warp-iteration, 16 warps per SM
+template <int NT, int NX>
+__global__ void __launch_bounds__(512, 1) tmemmix(int iters, float* out){
+  extern __shared__ double2 sm4[];
+  __shared__ unsigned tbase;
+  const int tid = threadIdx.x, warp = tid / 32;
+  if (warp == 0) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(&tbase)), "r"(512u) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+  }
+  __syncthreads();
+  asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+  const unsigned taddr = tbase + (((unsigned)(warp & 3) * 32u) << 16) + (unsigned)(warp / 4) * 64u;   // lane quarter of this warp, own columns
+  unsigned r[16];
+  #pragma unroll
+  for (int i = 0; i < 16; ++i) r[i] = tid * 16 + i;
+  double2 v[8];
+  #pragma unroll
+  for (int i = 0; i < 8; ++i) v[i] = make_double2(tid, i);
+  const unsigned base = (unsigned)__cvta_generic_to_shared(sm4 + tid);
+  for (int it = 0; it < iters; ++it) {
+    #pragma unroll
+    for (int u = 0; u < (NT > NX ? NT : NX); ++u) {
+      if (u < NX) asm volatile("st.shared.v2.f64 [%0], {%1, %2};" ::"r"(base + (u & 7) * 512 * 16), "d"(v[u & 7].x), "d"(v[u & 7].y) : "memory");
+      if (u < NT) {
+        asm volatile("tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16};"
+                     ::"r"(taddr + (u & 3) * 16), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]),
+                       "r"(r[8]), "r"(r[9]), "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15]) : "memory");
+        asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+        asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+                     : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
+                       "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+                     : "r"(taddr + ((u + 1) & 3) * 16) : "memory");
+        asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+      }
+      if (u < NX) asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v[(u + 3) & 7].x), "=d"(v[(u + 3) & 7].y) : "r"(base + ((u + 5) & 7) * 512 * 16) : "memory");
+    }
+  }
+  float s = 0;
+  #pragma unroll
+  for (int i = 0; i < 16; ++i) s += (float)r[i];
+  #pragma unroll
+  for (int i = 0; i < 8; ++i) s += (float)v[i].x + (float)v[i].y;
+  out[blockIdx.x * 512 + tid] = s;
+  __syncthreads();
+  if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tbase), "r"(512u) : "memory");
+}
+template <int NT, int NX> void run_tmem(double clock_hz){
+  float* out; CK(cudaMalloc(&out, 148 * 512 * 4));
+  const int smem = 512 * 8 * 16;
+  CK(cudaFuncSetAttribute(tmemmix<NT, NX>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+  const int iters = 2000;
+  float ms = timeit([&]{ tmemmix<NT, NX><<<148, 512, smem>>>(iters, out); }, 3);
+  CK(cudaGetLastError());
+  const double clk = ms * 1e-3 * clock_hz / iters;
+  printf("  tmem warps/SM=16 (tcgen05.st+ld x16) pairs=%d (lds+sts.128) pairs=%d per warp-iteration: %7.1f clk  -> tensor memory %4.0f B/clk/SM  (shared-memory pipe alone %4d clk)\n",
+         NT, NX, clk, NT ? 16.0 * NT * 4096 / clk : 0.0, 16 * NX * 2 * 4);
+  cudaFree(out);
+}
+
 int main(){
   cudaDeviceProp p; CK(cudaGetDeviceProperties(&p,0)); printf("%s SMs=%d L2=%d MB clock=%d MHz\n",p.name,p.multiProcessorCount,p.l2CacheSize>>20,p.clockRate/1000);
   size_t n=(size_t)1<<30; // 1 GiB
@@ -253,6 +315,7 @@ int main(){
     run_insm<double, 8192, 1, 0>("transform pair", hz); run_insm<float, 8192, 2, 0>("transform pair", hz);
     run_overlap<8, 0, 16>(hz); run_overlap<0, 8, 16>(hz); run_overlap<8, 8, 16>(hz); run_overlap<8, 8, 4>(hz);
     run_shfl<64, 0, 16>(hz); run_shfl<0, 8, 16>(hz); run_shfl<64, 8, 16>(hz);
+    run_tmem<8, 0>(hz); run_tmem<0, 8>(hz); run_tmem<8, 8>(hz);
   }
   return 0;
 }

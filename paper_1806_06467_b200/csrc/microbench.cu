@@ -278,6 +278,56 @@ template <int NT, int NX> void run_tmem(double clock_hz){
   cudaFree(out);
 }
 
+// which (lane, column) of tensor memory lands in which thread / register for the non-trivial tcgen05.ld shapes:
+// one warp writes value (lane << 16 | column) with 32x32b.x16 (thread = lane, register = column), reads it back with
+// 16x64b.x2, 16x128b.x2 and 16x256b.x1, and the host checks the formulas printed below
+__global__ void tmemprobe(unsigned* out){
+  __shared__ unsigned tbase;
+  const int t = threadIdx.x;
+  asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(&tbase)), "r"(32u) : "memory");
+  asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+  __syncwarp();
+  asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+  const unsigned ta = tbase;
+  unsigned w[16];
+  for (int c = 0; c < 16; ++c) w[c] = (t << 16) | c;
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16};"
+               ::"r"(ta), "r"(w[0]), "r"(w[1]), "r"(w[2]), "r"(w[3]), "r"(w[4]), "r"(w[5]), "r"(w[6]), "r"(w[7]),
+                 "r"(w[8]), "r"(w[9]), "r"(w[10]), "r"(w[11]), "r"(w[12]), "r"(w[13]), "r"(w[14]), "r"(w[15]) : "memory");
+  asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+  unsigned a[2], b[4], c[4];
+  asm volatile("tcgen05.ld.sync.aligned.16x64b.x2.b32 {%0, %1}, [%2];" : "=r"(a[0]), "=r"(a[1]) : "r"(ta) : "memory");
+  asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+  asm volatile("tcgen05.ld.sync.aligned.16x128b.x2.b32 {%0, %1, %2, %3}, [%4];" : "=r"(b[0]), "=r"(b[1]), "=r"(b[2]), "=r"(b[3]) : "r"(ta) : "memory");
+  asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+  asm volatile("tcgen05.ld.sync.aligned.16x256b.x1.b32 {%0, %1, %2, %3}, [%4];" : "=r"(c[0]), "=r"(c[1]), "=r"(c[2]), "=r"(c[3]) : "r"(ta) : "memory");
+  asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+  for (int i = 0; i < 2; ++i) out[t * 16 + i] = a[i];
+  for (int i = 0; i < 4; ++i) out[t * 16 + 4 + i] = b[i];
+  for (int i = 0; i < 4; ++i) out[t * 16 + 8 + i] = c[i];
+  __syncwarp();
+  asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tbase), "r"(32u) : "memory");
+}
+void run_tmemprobe(){
+  unsigned *d, h[32 * 16];
+  CK(cudaMalloc(&d, sizeof(h))); CK(cudaMemset(d, 0xff, sizeof(h)));
+  tmemprobe<<<1, 32>>>(d);
+  CK(cudaDeviceSynchronize());
+  CK(cudaMemcpy(h, d, sizeof(h), cudaMemcpyDeviceToHost));
+  bool ok64 = true, ok128 = true, ok256 = true;
+  for (int t = 0; t < 32; ++t) {
+    const int a = t / 4, c = t % 4;
+    for (int k = 0; k < 2; ++k) ok64 = ok64 && h[t * 16 + k] == (unsigned)(((a + 8 * (t & 1)) << 16) | ((c >> 1) + 2 * k));
+    for (int k = 0; k < 2; ++k) for (int e = 0; e < 2; ++e) ok128 = ok128 && h[t * 16 + 4 + 2 * k + e] == (unsigned)(((a + 8 * e) << 16) | (c + 4 * k));
+    for (int e = 0; e < 2; ++e) for (int i = 0; i < 2; ++i) ok256 = ok256 && h[t * 16 + 8 + 2 * e + i] == (unsigned)(((a + 8 * e) << 16) | (2 * c + i));
+  }
+  printf("  tmem shapes (thread t = 4a + c reads TMEM written by 32x32b with thread = lane, register = column):\n");
+  printf("    16x64b.x2 : register k     <- (lane a + 8*(t&1), column (c>>1) + 2k)      %s\n", ok64 ? "verified" : "MISMATCH");
+  printf("    16x128b.x2: register 2k+e  <- (lane a + 8e,      column c + 4k)           %s\n", ok128 ? "verified" : "MISMATCH");
+  printf("    16x256b.x1: register 2e+i  <- (lane a + 8e,      column 2c + i)           %s\n", ok256 ? "verified" : "MISMATCH");
+  cudaFree(d);
+}
+
 int main(){
   cudaDeviceProp p; CK(cudaGetDeviceProperties(&p,0)); printf("%s SMs=%d L2=%d MB clock=%d MHz\n",p.name,p.multiProcessorCount,p.l2CacheSize>>20,p.clockRate/1000);
   size_t n=(size_t)1<<30; // 1 GiB
@@ -316,6 +366,7 @@ int main(){
     run_overlap<8, 0, 16>(hz); run_overlap<0, 8, 16>(hz); run_overlap<8, 8, 16>(hz); run_overlap<8, 8, 4>(hz);
     run_shfl<64, 0, 16>(hz); run_shfl<0, 8, 16>(hz); run_shfl<64, 8, 16>(hz);
     run_tmem<8, 0>(hz); run_tmem<0, 8>(hz); run_tmem<8, 8>(hz);
+    run_tmemprobe();
   }
   return 0;
 }

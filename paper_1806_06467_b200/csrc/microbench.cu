@@ -134,6 +134,59 @@ template <typename T, int N, int G, int VAR, int GTX = -1> void run_insm(const c
   printf("  in-SM %-22s N=%d %s groups/SM=%d: %.3f clk/element/SM\n", what, N, sizeof(T) == 8 ? "f64" : "f32", G, ms * 1e-3 * clock_hz / iters / ((double)G * N));
   cudaFree(tw); cudaFree(out);
 }
+// two lines per thread group with ONE register set: a line lives in shared memory between its stages (gather ->
+// stage -> scatter per block, lines A and B alternating), so the exchange latency of one line lies under the
+// butterflies of the other.  Every transform here ends with one extra (natural-order) exchange that a real pass
+// would replace by its global load / store, so compare LINES = 2 with LINES = 1 of this same kernel.
+template <typename T, int N, int STAGE, int DIR, int GT>
+__device__ __forceinline__ void alt_block(typename fresnel::cplx_of<T>::type* buf, int j, const typename fresnel::cplx_of<T>::type* tw, int bar){
+  using namespace fresnel; using C = typename cplx_of<T>::type;
+  constexpr bool LAST = STAGE == fr_num_stages(N) - 1; constexpr int TL = N / 16;
+  C v[16];
+  fr_sync<GT>(bar);
+  fft_stage_gather<T, N, false, 1>(v, buf, 0, j);
+  fr_sync<GT>(bar);
+  fft_stage_compute<T, N, STAGE, DIR>(v, j, tw);
+  if constexpr (LAST) {
+    #pragma unroll
+    for (int r = 0; r < 16; ++r) buf[fr_pad(j + r * TL)] = v[r];
+  } else fft_stage_scatter<T, N, STAGE, false, 1>(v, buf, 0, j);
+}
+template <typename T, int N, int G, int LINES>
+__global__ void __launch_bounds__(G * (N / 16), 1) insm_alt(int iters, const typename fresnel::cplx_of<T>::type* tw, typename fresnel::cplx_of<T>::type* out){
+  using namespace fresnel; using C = typename cplx_of<T>::type;
+  constexpr int TL = N / 16, PL = fr_padded_len(N), S = fr_num_stages(N); constexpr int GT = G == 1 ? 0 : TL;
+  extern __shared__ __align__(16) unsigned char smraw[];
+  const int tid = threadIdx.x, grp = tid / TL, j = tid % TL;
+  C* bufA = reinterpret_cast<C*>(smraw) + (size_t)grp * PL * LINES; C* bufB = bufA + PL;
+  for (int r = 0; r < 16; ++r) { C z; z.x = (T)(tid + r) * (T)1e-3; z.y = (T)r; bufA[fr_pad(j + r * TL)] = z; if (LINES == 2) bufB[fr_pad(j + r * TL)] = z; }
+  fr_sync<GT>(1 + grp);
+  for (int it = 0; it < iters; ++it) {
+    int jj = j; asm volatile("" : "+r"(jj));
+    const C* t = tw; asm volatile("" : "+l"(t));
+#define FR_BOTH(STAGE, DIR) { alt_block<T, N, STAGE, DIR, GT>(bufA, jj, t, 1 + grp); if (LINES == 2) alt_block<T, N, STAGE, DIR, GT>(bufB, jj, t, 1 + grp); }
+    FR_BOTH(0, -1) FR_BOTH(1, -1) if constexpr (S > 2) FR_BOTH(2, -1) if constexpr (S > 3) FR_BOTH(3, -1)
+    asm volatile("" : "+l"(t));
+    FR_BOTH(0, +1) FR_BOTH(1, +1) if constexpr (S > 2) FR_BOTH(2, +1) if constexpr (S > 3) FR_BOTH(3, +1)
+#undef FR_BOTH
+  }
+  fr_sync<GT>(1 + grp);
+  C s = bufA[fr_pad(j)]; if (LINES == 2) s.x += bufB[fr_pad(j)].x;
+  out[blockIdx.x * blockDim.x + tid] = s;
+}
+template <typename T, int N, int G, int LINES> void run_alt(double clock_hz){
+  using C = typename fresnel::cplx_of<T>::type;
+  C *tw, *out; CK(cudaMalloc(&tw, 65536 * sizeof(C))); CK(cudaMemset(tw, 0, 65536 * sizeof(C))); CK(cudaMalloc(&out, 148 * 1024 * sizeof(C)));
+  const int smem = G * LINES * fresnel::fr_padded_len(N) * sizeof(C);
+  CK(cudaFuncSetAttribute(insm_alt<T, N, G, LINES>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+  const int iters = 300;
+  float ms = timeit([&]{ insm_alt<T, N, G, LINES><<<148, G * (N / 16), smem>>>(iters, tw, out); }, 3);
+  CK(cudaGetLastError());
+  printf("  in-SM lines in shared memory between stages, N=%d %s groups/SM=%d lines/group=%d: %.3f clk/element/SM\n", N, sizeof(T) == 8 ? "f64" : "f32", G, LINES,
+         ms * 1e-3 * clock_hz / iters / ((double)G * LINES * N));
+  cudaFree(tw); cudaFree(out);
+}
+
 // every warp interleaves NM*16 DFMA with NX (STS.128 + LDS.128) pairs per iteration, no barriers, thread-private slots
 template <int NM, int NX, int WARPS>
 __global__ void __launch_bounds__(WARPS * 32, 1) overlap(int iters, double* out){
@@ -363,6 +416,9 @@ int main(){
     run_insm<float, 2048, 8, 0, 32>("pair, warp-local sync", hz);
     run_insm<float, 4096, 4, 1>("butterflies", hz); run_insm<float, 4096, 4, 2>("exchanges", hz); run_insm<float, 4096, 4, 0>("transform pair", hz);
     run_insm<double, 8192, 1, 0>("transform pair", hz); run_insm<float, 8192, 2, 0>("transform pair", hz);
+    run_alt<double, 2048, 4, 1>(hz); run_alt<double, 2048, 3, 2>(hz); run_alt<double, 2048, 2, 2>(hz);
+    run_alt<double, 4096, 2, 1>(hz); run_alt<double, 4096, 1, 2>(hz);
+    run_alt<float, 2048, 8, 1>(hz); run_alt<float, 2048, 4, 2>(hz); run_alt<float, 4096, 4, 1>(hz); run_alt<float, 4096, 2, 2>(hz);
     run_overlap<8, 0, 16>(hz); run_overlap<0, 8, 16>(hz); run_overlap<8, 8, 16>(hz); run_overlap<8, 8, 4>(hz);
     run_shfl<64, 0, 16>(hz); run_shfl<0, 8, 16>(hz); run_shfl<64, 8, 16>(hz);
     run_tmem<8, 0>(hz); run_tmem<0, 8>(hz); run_tmem<8, 8>(hz);

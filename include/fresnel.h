@@ -22,13 +22,19 @@
  *              synchronising (except fresnel_plan_synchronize and plan create/destroy).  No device
  *              memory is allocated in the hot calls: the plan owns FFT twiddles, chirp tables and
  *              per-batch scalars.  All hot calls are CUDA-graph capturable.
- *   Errors:    return codes only, never exceptions or aborts.  On any error nothing is enqueued.
+ *   Errors:    return codes only, never exceptions or aborts.  Argument errors (INVALID_ARG, UNSUPPORTED) are
+ *              detected before anything is enqueued and leave the wavefront untouched -- for a whole train in
+ *              fresnel_system_run too.  FRESNEL_ERR_CUDA / FRESNEL_ERR_ALLOC raised by a launch in the middle of
+ *              a call (between the row and the column pass, or between two surfaces of a train) leave the
+ *              kernels enqueued so far in the stream: the wavefront contents are then unspecified.
  *                FRESNEL_ERR_INVALID_ARG  NULL plan/wf/host array, lambda <= 0, pixel <= 0, non-finite
  *                                         z, z == 0 where a division by z is needed, f == 0 or NaN,
  *                                         bad direction
  *                FRESNEL_ERR_UNSUPPORTED  N not a power of two in [64, 8192] (the paper's N = 2800
  *                                         run, is a later milestone), bad dtype
- *                FRESNEL_ERR_ALLOC        device/host allocation failed (plan create only)
+ *                FRESNEL_ERR_ALLOC        device/host allocation failed (plan create, fresnel_plan_reserve_tables),
+ *                                         or a call needs more chirp-table slots than are free (all taken by
+ *                                         captured graphs: see fresnel_plan_reserve_tables)
  *                FRESNEL_ERR_CUDA         a CUDA runtime call or launch failed
  *   Threads:   a plan is not thread-safe; distinct plans are independent.
  *   There is no CPU fallback: without a CUDA device plan creation fails with FRESNEL_ERR_CUDA.
@@ -63,8 +69,22 @@ enum { FRESNEL_FORWARD = +1, FRESNEL_INVERSE = -1 };
  * table cache.  N: power of two in [64, 8192]; batch >= 1.  *out is set only on FRESNEL_OK. */
 fresnel_status fresnel_plan_create(fresnel_plan **out, int N, int batch, fresnel_dtype dtype);
 
-/* Stream all later calls enqueue on (a cudaStream_t passed as void*; NULL = legacy default stream). */
+/* Stream all later calls enqueue on (a cudaStream_t passed as void*; NULL = legacy default stream).  The new
+ * stream is made to wait for everything the plan has enqueued on the old one (its cached tables were built and
+ * are read there); if either stream is being captured the cached tables are forgotten instead. */
 fresnel_status fresnel_plan_set_stream(fresnel_plan *p, void *cuda_stream);
+
+/* Chirp-table cache.  A plan owns a pool of 1-D table slots ([batch][N] complex each; 64 at creation) that cache
+ * the lens / Fresnel chirps, transfer functions and 1/lambda arrays by value, least recently used first out.
+ * fresnel_plan_reserve_tables makes sure at least n_tables slots are usable by eager calls (allocates device
+ * memory: not while the stream is being captured -> FRESNEL_ERR_UNSUPPORTED).  A fused train
+ * (fresnel_system_run) holds 2 tables per surface at once; longer trains than the pool allows are split.
+ * CUDA graphs: tables built while the stream is being captured belong to that graph from then on -- replays
+ * rewrite them, so they are never shared with eager calls nor evicted, only reused by later calls of the same
+ * capture.  After destroying such graphs, fresnel_plan_release_graph_tables returns their slots to the pool
+ * (replaying a graph captured before the release is then undefined). */
+fresnel_status fresnel_plan_reserve_tables(fresnel_plan *p, int n_tables);
+fresnel_status fresnel_plan_release_graph_tables(fresnel_plan *p);
 
 /* Block the host until everything enqueued on the plan's stream has finished. */
 fresnel_status fresnel_plan_synchronize(fresnel_plan *p);
@@ -81,6 +101,24 @@ fresnel_status fresnel_plan_launch_count(const fresnel_plan *p, unsigned long lo
  * pass, events[1] between the passes and events[2] after its column pass, on the plan's stream.
  * events: HOST array of 3 cudaEvent_t handles owned by the caller (passed as void*); NULL disarms. */
 fresnel_status fresnel_plan_record_pass_events(fresnel_plan *p, void *const events[3]);
+
+/* Profiling hooks of fresnel_system_run (used by bench.py for the per-kernel durations behind `roofline`).
+ * fresnel_plan_record_train_events: the NEXT fresnel_system_run records events[k] right before its k-th pass
+ * kernel and one more event after the last one (as far as n_events reaches), on the plan's stream; events are
+ * cudaEvent_t handles owned by the caller; n_events = 0 disarms.  An event between two kernels switches off
+ * their programmatic launch overlap, so instrumented trains run a few per cent slower.
+ * fresnel_plan_last_schedule: the pass kernels the last fresnel_system_run enqueued, in order: direction
+ * (0 along rows, 1 along columns), convolutions per resident line (0: a plain transform pass of direct Fresnel
+ * or an optic-only pass, 1, or 2 for a fused pass), the surface whose optic the pass applied (or whose
+ * propagation it finished), and the number of real N x N maps it read.  *count receives the total. */
+typedef struct {
+    int direction;
+    int convolutions;
+    int first_surface;
+    int maps_read;
+} fresnel_pass_info;
+fresnel_status fresnel_plan_record_train_events(fresnel_plan *p, void *const *events, int n_events);
+fresnel_status fresnel_plan_last_schedule(const fresnel_plan *p, fresnel_pass_info *out, int capacity, int *count);
 
 /* ---- the operations of the hot path ----------------------------------------------------------- */
 
@@ -138,7 +176,14 @@ fresnel_status fresnel_surface_as(fresnel_plan *p, void *wf, const double *pixel
  * z == 0 applies the optic only.  pixel_inout (HOST, length batch) carries the running pixel pitch and holds the
  * final one on return; method_used (HOST, length nsurf, may be NULL) receives 0 / 1, or -1 where z == 0.
  * All surfaces are validated before anything is enqueued; the calls enqueue only, so a train can be captured
- * into one CUDA graph. */
+ * into one CUDA graph.
+ * TRAIN-LEVEL FUSION.  The row and the column convolution of an angular-spectrum step commute, so a run of L
+ * consecutive angular-spectrum surfaces is scheduled as
+ *     rows_0 (optic_0 on load) | cols_0, optic_1, cols_1 | rows_1, optic_2, rows_2 | ... | last convolution:
+ * L+1 passes over the wavefront instead of 2L, every inner pass holding each line on chip through
+ * convolution -> optic of the next surface -> convolution ("10 optics ... 19 FFT" become 11 passes).
+ * Column passes fetch the optic's map tiles by TMA.  Results equal the surface-by-surface order up to rounding
+ * (the two orders differ by the commuted convolutions only).  Direct-Fresnel and z == 0 surfaces end a run. */
 typedef struct {
     double f;
     const void *amp;
@@ -172,7 +217,7 @@ fresnel_status fresnel_memcpy_d2h(fresnel_plan *p, void *dst_host, const void *s
 
 const char *fresnel_status_string(fresnel_status s);
 
-/* Library build string, e.g. "fresnel-b200 0.1 sm_100a". */
+/* Library build string, e.g. "fresnel-b200 0.2 sm_100a". */
 const char *fresnel_version(void);
 
 #ifdef __cplusplus

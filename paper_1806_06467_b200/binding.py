@@ -27,7 +27,8 @@ C64, C128 = 0, 1
 # every symbol include/fresnel.h declares (tests/test_abi.py checks the header against this list)
 SYMBOLS = (
     "fresnel_plan_create", "fresnel_plan_set_stream", "fresnel_plan_synchronize", "fresnel_plan_destroy",
-    "fresnel_plan_launch_count", "fresnel_plan_record_pass_events", "fresnel_apply_qpf", "fresnel_apply_mask", "fresnel_fft2d",
+    "fresnel_plan_launch_count", "fresnel_plan_record_pass_events", "fresnel_plan_record_train_events",
+    "fresnel_plan_last_schedule", "fresnel_plan_reserve_tables", "fresnel_plan_release_graph_tables", "fresnel_apply_qpf", "fresnel_apply_mask", "fresnel_fft2d",
     "fresnel_propagate_as", "fresnel_propagate_direct", "fresnel_surface_as", "fresnel_system_run", "fresnel_accumulate_intensity", "fresnel_memcpy_h2d",
     "fresnel_memcpy_d2h", "fresnel_status_string", "fresnel_version",
 )
@@ -40,6 +41,11 @@ METHOD_AS, METHOD_DIRECT, METHOD_AUTO = 0, 1, 2
 class _Surface(ctypes.Structure):       # fresnel_surface of include/fresnel.h
     _fields_ = [("f", ctypes.c_double), ("amp", ctypes.c_void_p), ("opd", ctypes.c_void_p),
                 ("z", ctypes.c_double), ("method", ctypes.c_int)]
+
+
+class _PassInfo(ctypes.Structure):      # fresnel_pass_info of include/fresnel.h
+    _fields_ = [("direction", ctypes.c_int), ("convolutions", ctypes.c_int), ("first_surface", ctypes.c_int),
+                ("maps_read", ctypes.c_int)]
 
 
 class FresnelError(RuntimeError):
@@ -65,6 +71,10 @@ def lib() -> ctypes.CDLL:
     L.fresnel_plan_destroy.argtypes = [vp]
     L.fresnel_plan_launch_count.argtypes = [vp, ctypes.POINTER(ctypes.c_ulonglong)]
     L.fresnel_plan_record_pass_events.argtypes = [vp, ctypes.POINTER(vp)]
+    L.fresnel_plan_record_train_events.argtypes = [vp, ctypes.POINTER(vp), ci]
+    L.fresnel_plan_last_schedule.argtypes = [vp, ctypes.POINTER(_PassInfo), ci, ctypes.POINTER(ci)]
+    L.fresnel_plan_reserve_tables.argtypes = [vp, ci]
+    L.fresnel_plan_release_graph_tables.argtypes = [vp]
     L.fresnel_apply_qpf.argtypes = [vp, vp, dp, dp, cd]
     L.fresnel_apply_mask.argtypes = [vp, vp, vp, vp, dp]
     L.fresnel_fft2d.argtypes = [vp, vp, ci, ci]
@@ -138,6 +148,33 @@ class Plan:
                 e.record(self._stream)
         arr = (ctypes.c_void_p * 3)(*[ctypes.c_void_p(e.cuda_event) for e in events])
         self._chk(lib().fresnel_plan_record_pass_events(self._h, arr), "fresnel_plan_record_pass_events")
+
+    def record_train_events(self, events) -> None:
+        """Arm the train profiling hook: the next system_run records events[k] before its k-th pass kernel and one
+        more after the last (torch.cuda.Event(enable_timing=True) objects; None or [] disarms)."""
+        if not events:
+            self._chk(lib().fresnel_plan_record_train_events(self._h, None, 0), "fresnel_plan_record_train_events")
+            return
+        for e in events:
+            if not e.cuda_event:
+                e.record(self._stream)
+        arr = (ctypes.c_void_p * len(events))(*[ctypes.c_void_p(e.cuda_event) for e in events])
+        self._chk(lib().fresnel_plan_record_train_events(self._h, arr, len(events)), "fresnel_plan_record_train_events")
+
+    def last_schedule(self):
+        """Pass kernels of the last system_run: list of dicts (direction, convolutions, first_surface, maps_read)."""
+        n = ctypes.c_int(0)
+        self._chk(lib().fresnel_plan_last_schedule(self._h, None, 0, ctypes.byref(n)), "fresnel_plan_last_schedule")
+        arr = (_PassInfo * max(n.value, 1))()
+        self._chk(lib().fresnel_plan_last_schedule(self._h, arr, n.value, ctypes.byref(n)), "fresnel_plan_last_schedule")
+        return [{"direction": arr[i].direction, "convolutions": arr[i].convolutions,
+                 "first_surface": arr[i].first_surface, "maps_read": arr[i].maps_read} for i in range(n.value)]
+
+    def reserve_tables(self, n: int) -> None:
+        self._chk(lib().fresnel_plan_reserve_tables(self._h, int(n)), "fresnel_plan_reserve_tables")
+
+    def release_graph_tables(self) -> None:
+        self._chk(lib().fresnel_plan_release_graph_tables(self._h), "fresnel_plan_release_graph_tables")
 
     def close(self) -> None:
         if getattr(self, "_h", None) is not None and self._h.value:

@@ -75,13 +75,12 @@ def build(force: bool = False, verbose: bool = False) -> str:
 
 
 def build_microbench() -> str:
-    """The stand-alone measurement tools of csrc/microbench.cu and csrc/microbench_tmem_fft.cu (DESIGN.md,
-    profiles/r01_microbench.txt)."""
+    """The stand-alone roof measurements of csrc/microbench.cu (HBM copy, DFMA/FFMA rates, in-SM rates of the
+    transform code): the numbers bench.py's `roofline.alu` and DESIGN.md quote (profiles/r01_microbench.txt)."""
     out = os.path.join(HERE, "microbench")
-    for name in ("microbench", "microbench_tmem_fft"):
-        cmd = [_nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "--expt-relaxed-constexpr",
-               "-o", os.path.join(HERE, name), os.path.join(CSRC, name + ".cu")]
-        subprocess.run(cmd, check=True)
+    cmd = [_nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "--expt-relaxed-constexpr",
+           "-o", out, os.path.join(CSRC, "microbench.cu")]
+    subprocess.run(cmd, check=True)
     return out
 
 

@@ -41,6 +41,11 @@ FR_DEV void tma_load_3d(void *dst, const CUtensorMap *map, uint64_t *bar, int x,
     asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
                  ::"r"(smem_u32(dst)), "l"(map), "r"(smem_u32(bar)), "r"(x), "r"(y), "r"(z) : "memory");
 }
+FR_DEV void tma_load_2d(void *dst, const CUtensorMap *map, uint64_t *bar, int x, int y)
+{
+    asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
+                 ::"r"(smem_u32(dst)), "l"(map), "r"(smem_u32(bar)), "r"(x), "r"(y) : "memory");
+}
 FR_DEV void tma_store_3d(const CUtensorMap *map, const void *src, int x, int y, int z)
 {
     asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.bulk_group [%0, {%2, %3, %4}], [%1];"
@@ -70,9 +75,33 @@ template <int ROW_BYTES> FR_DEV uint32_t tile_swizzle(uint32_t off)
 
 constexpr int kTmaBoxRows = 256;
 
+// Column tile of a REAL [N][N] surface map, fetched in the middle of a fused kernel (MODE_CONV2) into the exchange
+// space while it is idle: rows of max(W * sizeof(T), 16) bytes (the TMA minimum), no swizzle.  Every thread then
+// picks up its 16 entries (rows j + r*TL of column g).
+template <typename T, int W> struct MapTile {
+    static constexpr int ROW_BYTES = (W * (int)sizeof(T) < 16) ? 16 : W * (int)sizeof(T);
+    static constexpr int BOX_COLS = ROW_BYTES / (int)sizeof(T);
+};
+
+template <typename T, int N, int W>
+FR_DEV void fetch_map_tile(unsigned char *tile, const CUtensorMap *mmap, uint64_t *bar, uint32_t &parity, int col0, int tid)
+{
+    using MT = MapTile<T, W>;
+    fence_async_proxy();                             // the exchange traffic (generic proxy) is ordered before the TMA writes
+    __syncthreads();                                 // every group is done with the exchange space
+    if (tid == 0) {
+        mbar_expect_tx(bar, (uint32_t)(N * MT::ROW_BYTES));
+#pragma unroll 1
+        for (int r0 = 0; r0 < N; r0 += kTmaBoxRows) tma_load_2d(tile + (size_t)r0 * MT::ROW_BYTES, mmap, bar, col0, r0);
+    }
+    mbar_wait(bar, parity);
+    parity ^= 1u;
+}
+
 template <typename T, int N, int W, int MODE, int MINB>
 __global__ void __launch_bounds__(W *(N / 16), MINB)
-col_tma_kernel(PassArgs<T> a, const __grid_constant__ CUtensorMap tmap)
+col_tma_kernel(PassArgs<T> a, const __grid_constant__ CUtensorMap tmap, const __grid_constant__ CUtensorMap tmap_amp2,
+               const __grid_constant__ CUtensorMap tmap_opd2)
 {
     using C = typename cplx_of<T>::type;
     constexpr int TL = N / 16;                       // threads per column
@@ -134,10 +163,56 @@ col_tma_kernel(PassArgs<T> a, const __grid_constant__ CUtensorMap tmap)
 #pragma unroll
         for (int r = 0; r < 16; ++r) v[r] = cmul(v[r], ldg_c(m + j + r * TL));
     }
-    if constexpr (MODE == MODE_CONV) fft_line<T, N, +1, false, W, GT>(v, buf, g, j, a.tw, 1 + g);
+    if constexpr (MODE == MODE_CONV || MODE == MODE_CONV2) fft_line<T, N, +1, false, W, GT>(v, buf, g, j, a.tw, 1 + g);
     if (a.scale != (T)1) {
 #pragma unroll
         for (int r = 0; r < 16; ++r) { v[r].x *= a.scale; v[r].y *= a.scale; }
+    }
+    if constexpr (MODE == MODE_CONV2) {
+        // the optic of the next surface on the resident tile (its maps arrive by TMA in the exchange space, which is
+        // idle between the two convolutions), then that surface's column convolution
+        using MT = MapTile<T, W>;
+        uint32_t parity = 1;                         // phase 0 was the wavefront tile
+        if (a.opd2 != nullptr) {
+            fetch_map_tile<T, N, W>(tile, &tmap_opd2, &full_bar, parity, col0, tid);
+            const T il = (T)a.inv_lambda[b];
+            T u[16];
+            bool all_small = true;
+#pragma unroll
+            for (int r = 0; r < 16; ++r) {
+                u[r] = *reinterpret_cast<const T *>(tile + (size_t)(j + r * TL) * MT::ROW_BYTES + g * sizeof(T)) * il;
+                all_small = all_small && phasor_is_small(u[r]);
+            }
+            if (all_small) {
+#pragma unroll
+                for (int r = 0; r < 16; ++r) v[r] = cmul(v[r], phasor_turns_small(u[r]));
+            } else {
+#pragma unroll
+                for (int r = 0; r < 16; ++r) v[r] = cmul(v[r], phasor_turns_any(u[r]));
+            }
+        }
+        if (a.amp2 != nullptr) {
+            fetch_map_tile<T, N, W>(tile, &tmap_amp2, &full_bar, parity, col0, tid);
+#pragma unroll
+            for (int r = 0; r < 16; ++r) {
+                const T s = *reinterpret_cast<const T *>(tile + (size_t)(j + r * TL) * MT::ROW_BYTES + g * sizeof(T));
+                v[r].x *= s; v[r].y *= s;
+            }
+        }
+        if (a.opd2 != nullptr || a.amp2 != nullptr) __syncthreads();      // the map tile has been read: exchange space again
+        if (a.lens2 != nullptr) {
+            const C *l = a.lens2 + (size_t)b * N;
+            const C c = ldg_c(l + col0 + g);
+#pragma unroll
+            for (int r = 0; r < 16; ++r) v[r] = cmul(v[r], cmul(ldg_c(l + j + r * TL), c));
+        }
+        fft_line<T, N, -1, false, W, GT>(v, buf, g, j, a.tw, 1 + g);
+        {
+            const C *m = a.mid2 + (size_t)b * N;
+#pragma unroll
+            for (int r = 0; r < 16; ++r) v[r] = cmul(v[r], ldg_c(m + j + r * TL));
+        }
+        fft_line<T, N, +1, false, W, GT>(v, buf, g, j, a.tw, 1 + g);
     }
 
     __syncthreads();                                 // every group is done with its exchange buffer
@@ -186,24 +261,27 @@ template <typename T, int N> struct ColTmaGeom {
     static constexpr bool supported = TL >= 32;      // named barriers work on whole warps
 };
 
+// tmap: the wavefront; tmap_amp2 / tmap_opd2: the maps of the in-between optic (MODE_CONV2; read only when
+// a.amp2 / a.opd2 are non-null, any valid tensor map otherwise)
 template <typename T, int N, int MODE>
-cudaError_t launch_col_tma(const PassArgs<T> &a, const CUtensorMap &tmap, int batch, cudaStream_t stream)
+cudaError_t launch_col_tma(const PassArgs<T> &a, const CUtensorMap &tmap, const CUtensorMap &tmap_amp2, const CUtensorMap &tmap_opd2,
+                           int batch, cudaStream_t stream)
 {
     using G = ColTmaGeom<T, N>;
     if constexpr (!G::supported) {
         return cudaErrorNotSupported;
     } else {
         auto kern = col_tma_kernel<T, N, G::W, MODE, G::MINB>;
-        static bool configured = false;
-        if (!configured) {
+        static std::atomic<unsigned long long> configured{0};
+        if (fr_needs_configuring(configured)) {
             cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::smem + 1024);
             if (e != cudaSuccess) return e;
-            configured = true;
+            fr_mark_configured(configured);
         }
         dim3 grid(N / G::W, batch, 1);
         PassArgs<T> b = a;
         if (b.prefetch_distance < 0) b.prefetch_distance = -b.prefetch_distance * G::MINB;
-        return launch_pdl(kern, grid, dim3(G::threads), G::smem + 1024, stream, b.pdl != 0, b, tmap);
+        return launch_pdl(kern, grid, dim3(G::threads), G::smem + 1024, stream, b.pdl != 0, b, tmap, tmap_amp2, tmap_opd2);
     }
 }
 

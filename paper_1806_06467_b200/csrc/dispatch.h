@@ -8,8 +8,12 @@ namespace fresnel {
 #define FR_DECL(N)                                                                                              \
     cudaError_t launch_pass_f32_##N(bool col, int mode, const PassArgs<float> &a, int batch, cudaStream_t s);  \
     cudaError_t launch_pass_f64_##N(bool col, int mode, const PassArgs<double> &a, int batch, cudaStream_t s);   \
-    cudaError_t launch_col_tma_f32_##N(int mode, const PassArgs<float> &a, const CUtensorMap &m, int batch, cudaStream_t s);   \
-    cudaError_t launch_col_tma_f64_##N(int mode, const PassArgs<double> &a, const CUtensorMap &m, int batch, cudaStream_t s);   \
+    cudaError_t launch_col_tma_f32_##N(int mode, const PassArgs<float> &a, const CUtensorMap &m, const CUtensorMap &ma,        \
+                                       const CUtensorMap &mo, int batch, cudaStream_t s);                                       \
+    cudaError_t launch_col_tma_f64_##N(int mode, const PassArgs<double> &a, const CUtensorMap &m, const CUtensorMap &ma,       \
+                                       const CUtensorMap &mo, int batch, cudaStream_t s);                                       \
+    int col_tma_map_box_f32_##N();                                                                              \
+    int col_tma_map_box_f64_##N();                                                                              \
     int col_tma_width_f32_##N();                                                                                \
     int col_tma_width_f64_##N();
 FR_DECL(64) FR_DECL(128) FR_DECL(256) FR_DECL(512) FR_DECL(1024) FR_DECL(2048) FR_DECL(4096) FR_DECL(8192)

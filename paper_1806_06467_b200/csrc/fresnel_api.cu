@@ -1,6 +1,6 @@
-// fresnel_api.cu -- the C ABI of include/fresnel.h: argument checks, chirp-table cache, launches.
-// Every step of the hot path runs in the kernels of pass_kernel.cuh / pointwise.cuh / tables.cuh;
-// this file only decides which tables a call needs and enqueues the passes.
+// fresnel_api.cu -- the C ABI of include/fresnel.h: argument checks, chirp-table cache, pass scheduling, launches.
+// Every step of the hot path runs in the kernels of pass_kernel.cuh / col_tma.cuh / pointwise.cuh / tables.cuh;
+// this file only decides which tables a call needs, in which order the passes run, and enqueues them.
 #include <cmath>
 #include <cstdint>
 #include <cstdlib>
@@ -20,21 +20,44 @@ using namespace fresnel;
 
 namespace {
 
-constexpr int kSlots = 64;              // cached chirp tables per plan (a 20-surface train needs 40)
+constexpr int kDefaultSlots = 64;       // table slots of a new plan (fresnel_plan_reserve_tables grows the pool)
+constexpr int kMaxMapDescs = 64;        // cached tensor maps of surface maps (fused column passes)
 const long double PI_L = 3.14159265358979323846264338327950288419716939937510L;
 
+// kinds of cached 1-D tables
+enum { KIND_CENTRED = 0, KIND_FFTORDER = 1, KIND_SCALARS = 2 };
+
+// One cached table: [batch][N] complex of the plan's dtype (chirps) or [batch] doubles (KIND_SCALARS: 1/lambda).
+// Ownership.  An EAGER slot serves cache hits and may be evicted (least recently used).  A slot written while the
+// stream is being captured into a CUDA graph is GRAPH-OWNED from then on: the builder was only recorded, and every
+// replay rewrites the slot behind the host's back -- so it never serves an eager hit and is never evicted; it
+// serves hits only to later calls of the SAME capture (its builder node precedes them in that graph).  Graph-owned
+// slots return to the pool with fresnel_plan_release_graph_tables.
 struct TableSlot {
     void *dev = nullptr;
     bool valid = false;
+    bool graph_owned = false;
+    unsigned long long capture_id = 0;
     uint64_t stamp = 0;
-    uint64_t pinned_call = 0;           // API call that last asked for it (never evicted within that call)
-    int index_mode = 0, alt_sign = 0;
+    uint64_t pin = 0;                   // pin epoch that last asked for it (never evicted within that epoch)
+    int kind = 0, alt_sign = 0;
     std::vector<ChirpSpec> key;
 };
 
 struct TableRequest {
-    int slot;
-    bool build;
+    int slot = -1;                      // -1: no slot could be had (all graph-owned or pinned)
+    bool build = false;
+};
+
+struct CaptureState {
+    bool active = false;
+    unsigned long long id = 0;
+};
+
+struct MapDesc {
+    const void *ptr = nullptr;
+    uint64_t stamp = 0;
+    CUtensorMap map{};
 };
 
 } // namespace
@@ -42,28 +65,49 @@ struct TableRequest {
 struct fresnel_plan {
     int N = 0, batch = 0;
     fresnel_dtype dtype = FRESNEL_C128;
+    int device = 0;                     // the CUDA device the plan lives on; every entry point switches to it
     cudaStream_t stream = nullptr;
+    cudaEvent_t order_ev = nullptr;     // orders the old and the new stream in fresnel_plan_set_stream
     void *tw = nullptr;                 // FFT twiddles
-    double *scal_dev = nullptr;         // [batch] 1/lambda
-    std::vector<double> scal_key;
-    bool scal_valid = false;
-    TableSlot slots[kSlots];
-    uint64_t clock = 0, call_id = 0;
+    std::vector<TableSlot> slots;
+    std::vector<void *> arenas;         // device allocations behind the slots
+    uint64_t clock = 0, pin_epoch = 0;
     unsigned long long launches = 0;
     int prefetch = 0;                   // L2 prefetch distance in tiles (see pass_kernel.cuh)
     int tma_w = 0;                      // columns per TMA tile of the column pass (0: not used for this N)
+    int map_box = 0;                    // columns per TMA box of a surface map (fused column pass)
     int sms = 148;
     int pdl = 1;                        // programmatic dependent launch of the pass kernels (FRESNEL_PDL=0: off, A/B timing)
+    int fuse = 1;                       // train-level pass fusion in fresnel_system_run (FRESNEL_FUSE=0: off, A/B timing)
     CUtensorMap tmap{};                  // tensor map of the wavefront last seen by the column pass
     const void *tmap_wf = nullptr;
+    std::vector<MapDesc> map_descs;     // tensor maps of surface maps, by pointer
     cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};   // profiling hook, see fresnel_plan_record_pass_events
     bool ev_armed = false;
+    std::vector<cudaEvent_t> train_ev;  // profiling hook, see fresnel_plan_record_train_events
+    std::vector<fresnel_pass_info> schedule;           // pass kernels of the last fresnel_system_run
     size_t esize() const { return dtype == FRESNEL_C128 ? sizeof(double2) : sizeof(float2); }
+    size_t slot_bytes() const { return (size_t)batch * N * esize(); }
 };
 
 namespace {
 
 bool is_pow2(int n) { return n > 0 && (n & (n - 1)) == 0; }
+
+// Every entry point runs on the plan's device, whatever the caller's current device is.
+struct DeviceGuard {
+    int prev = -1;
+    bool switched = false;
+    explicit DeviceGuard(const fresnel_plan *p)
+    {
+        if (cudaGetDevice(&prev) != cudaSuccess) { cudaGetLastError(); prev = -1; return; }
+        if (prev != p->device && cudaSetDevice(p->device) == cudaSuccess) switched = true;
+    }
+    ~DeviceGuard()
+    {
+        if (switched) cudaSetDevice(prev);
+    }
+};
 
 // ---- FFT twiddle tables (host, long double) --------------------------------------------------------
 template <typename C> void fill_twiddles_for(int N, std::vector<C> &out)
@@ -112,89 +156,131 @@ ChirpSpec make_spec(long double c_turns, double amp, double phase0)
     return s;
 }
 
-bool capturing(fresnel_plan *p)
+CaptureState capture_state(fresnel_plan *p)
 {
+    CaptureState c;
     cudaStreamCaptureStatus st = cudaStreamCaptureStatusNone;
-    if (cudaStreamIsCapturing(p->stream, &st) != cudaSuccess) { cudaGetLastError(); return false; }
-    return st != cudaStreamCaptureStatusNone;
+    unsigned long long id = 0;
+    if (cudaStreamGetCaptureInfo(p->stream, &st, &id) != cudaSuccess) { cudaGetLastError(); return c; }
+    c.active = st != cudaStreamCaptureStatusNone;
+    c.id = id;
+    return c;
 }
 
-// Find or allocate a cache slot for a table.  While the stream is being captured into a CUDA graph
-// the table is always rebuilt inside the graph, so that replays are self-contained.
-TableRequest request_table(fresnel_plan *p, int index_mode, int alt_sign, const std::vector<ChirpSpec> &key, bool force)
+// Grow the slot pool by `extra` slots (one device allocation).  Never called while capturing.
+fresnel_status grow_slots(fresnel_plan *p, int extra)
 {
-    ++p->clock;
-    for (int i = 0; i < kSlots; ++i) {
-        TableSlot &s = p->slots[i];
-        if (s.valid && s.index_mode == index_mode && s.alt_sign == alt_sign && s.key.size() == key.size() &&
-            std::memcmp(s.key.data(), key.data(), key.size() * sizeof(ChirpSpec)) == 0) {
-            s.stamp = p->clock;
-            s.pinned_call = p->call_id;
-            return {i, force};
-        }
-    }
-    // miss: take a free slot, else the least recently used one that this call has not asked for
-    int victim = -1;
-    for (int i = 0; i < kSlots && victim < 0; ++i)
-        if (!p->slots[i].valid) victim = i;
-    if (victim < 0)
-        for (int i = 0; i < kSlots; ++i) {
-            if (p->slots[i].pinned_call == p->call_id) continue;
-            if (victim < 0 || p->slots[i].stamp < p->slots[victim].stamp) victim = i;
-        }
-    TableSlot &s = p->slots[victim];
-    s.valid = true;
-    s.index_mode = index_mode;
-    s.alt_sign = alt_sign;
-    s.key = key;
-    s.stamp = p->clock;
-    s.pinned_call = p->call_id;
-    return {victim, true};
-}
-
-// Launch the builder for every requested table that is not cached (and the per-batch scalars).
-fresnel_status flush_builds(fresnel_plan *p, const TableRequest *req, int nreq, const double *scal /*or null*/)
-{
-    int build_idx[kBuildMaxTables];
-    int nb_tab = 0;
-    for (int i = 0; i < nreq; ++i)
-        if (req[i].build) build_idx[nb_tab++] = req[i].slot;
-    if (nb_tab == 0 && scal == nullptr) return FRESNEL_OK;
-    for (int b0 = 0; b0 < p->batch; b0 += kBuildMaxBatch) {
-        BuildArgs a;
-        std::memset(&a, 0, sizeof(a));
-        a.N = p->N;
-        a.b0 = b0;
-        a.nb = (p->batch - b0 < kBuildMaxBatch) ? p->batch - b0 : kBuildMaxBatch;
-        a.ntab = nb_tab;
-        a.is_double = p->dtype == FRESNEL_C128;
-        a.scal_out = scal ? p->scal_dev : nullptr;
-        for (int b = 0; b < a.nb; ++b) {
-            if (scal) a.scal[b] = scal[b0 + b];
-            for (int t = 0; t < nb_tab; ++t) a.t[t].spec[b] = p->slots[build_idx[t]].key[b0 + b];
-        }
-        for (int t = 0; t < nb_tab; ++t) {
-            a.t[t].out = p->slots[build_idx[t]].dev;
-            a.t[t].index_mode = p->slots[build_idx[t]].index_mode;
-            a.t[t].alt_sign = p->slots[build_idx[t]].alt_sign;
-        }
-        dim3 grid((p->N + 127) / 128, a.nb, nb_tab > 0 ? nb_tab : 1);
-        build_tables_kernel<<<grid, 128, 0, p->stream>>>(a);
-        if (cudaGetLastError() != cudaSuccess) return FRESNEL_ERR_CUDA;
-        ++p->launches;
+    if (extra <= 0) return FRESNEL_OK;
+    void *arena = nullptr;
+    if (cudaMalloc(&arena, (size_t)extra * p->slot_bytes()) != cudaSuccess) { cudaGetLastError(); return FRESNEL_ERR_ALLOC; }
+    p->arenas.push_back(arena);
+    for (int i = 0; i < extra; ++i) {
+        TableSlot s;
+        s.dev = (unsigned char *)arena + (size_t)i * p->slot_bytes();
+        p->slots.push_back(std::move(s));
     }
     return FRESNEL_OK;
 }
 
-// 1/lambda per batch element on the device (needed by the optic phasor); cached by value.
-const double *need_inv_lambda(fresnel_plan *p, const double *lambda, std::vector<double> &tmp, bool force)
+int eager_slot_count(const fresnel_plan *p)
 {
-    tmp.resize(p->batch);
-    for (int b = 0; b < p->batch; ++b) tmp[b] = (double)(1.0L / (long double)lambda[b]);
-    if (!force && p->scal_valid && p->scal_key == tmp) return nullptr;      // already resident
-    p->scal_key = tmp;
-    p->scal_valid = true;
-    return tmp.data();
+    int n = 0;
+    for (const TableSlot &s : p->slots)
+        if (!s.graph_owned) ++n;
+    return n;
+}
+
+// Find or assign a cache slot for a table (see TableSlot for the ownership rules).
+TableRequest request_table(fresnel_plan *p, int kind, int alt_sign, const std::vector<ChirpSpec> &key, const CaptureState &cap)
+{
+    ++p->clock;
+    const int ns = (int)p->slots.size();
+    for (int i = 0; i < ns; ++i) {
+        TableSlot &s = p->slots[i];
+        if (!s.valid || s.kind != kind || s.alt_sign != alt_sign || s.key.size() != key.size()) continue;
+        if (cap.active ? !(s.graph_owned && s.capture_id == cap.id) : s.graph_owned) continue;
+        if (std::memcmp(s.key.data(), key.data(), key.size() * sizeof(ChirpSpec)) != 0) continue;
+        s.stamp = p->clock;
+        s.pin = p->pin_epoch;
+        return {i, false};
+    }
+    // miss: a slot never used, else the least recently used eager slot that this pin epoch has not asked for
+    int victim = -1;
+    for (int i = 0; i < ns && victim < 0; ++i)
+        if (!p->slots[i].valid && !p->slots[i].graph_owned) victim = i;
+    if (victim < 0)
+        for (int i = 0; i < ns; ++i) {
+            const TableSlot &s = p->slots[i];
+            if (s.graph_owned || s.pin == p->pin_epoch) continue;
+            if (victim < 0 || s.stamp < p->slots[victim].stamp) victim = i;
+        }
+    if (victim < 0) return {-1, false};
+    TableSlot &s = p->slots[victim];
+    s.valid = true;
+    s.graph_owned = cap.active;
+    s.capture_id = cap.id;
+    s.kind = kind;
+    s.alt_sign = alt_sign;
+    s.key = key;
+    s.stamp = p->clock;
+    s.pin = p->pin_epoch;
+    return {victim, true};
+}
+
+// 1/lambda per batch element on the device (needed by the optic phasor): a KIND_SCALARS table.
+TableRequest request_inv_lambda(fresnel_plan *p, const double *lambda, const CaptureState &cap)
+{
+    std::vector<ChirpSpec> key(p->batch);
+    for (int b = 0; b < p->batch; ++b) key[b] = make_spec((long double)(double)(1.0L / (long double)lambda[b]), 0.0, 0.0);
+    return request_table(p, KIND_SCALARS, 0, key, cap);
+}
+
+// Launch the builder for every requested table that is not resident.
+fresnel_status flush_builds(fresnel_plan *p, const TableRequest *req, int nreq)
+{
+    std::vector<int> todo;
+    for (int i = 0; i < nreq; ++i) {
+        if (req[i].slot < 0) return FRESNEL_ERR_ALLOC;
+        if (!req[i].build) continue;
+        bool dup = false;
+        for (int s : todo) dup = dup || s == req[i].slot;
+        if (!dup) todo.push_back(req[i].slot);
+    }
+    // scalar tables ride along one per launch; chirp tables kBuildMaxTables per launch
+    std::vector<int> chirps, scalars;
+    for (int s : todo) (p->slots[s].kind == KIND_SCALARS ? scalars : chirps).push_back(s);
+    size_t ci = 0, si = 0;
+    while (ci < chirps.size() || si < scalars.size()) {
+        const int ntab = (int)((chirps.size() - ci < (size_t)kBuildMaxTables) ? chirps.size() - ci : (size_t)kBuildMaxTables);
+        const int sc = si < scalars.size() ? scalars[si] : -1;
+        for (int b0 = 0; b0 < p->batch; b0 += kBuildMaxBatch) {
+            BuildArgs a;
+            std::memset(&a, 0, sizeof(a));
+            a.N = p->N;
+            a.b0 = b0;
+            a.nb = (p->batch - b0 < kBuildMaxBatch) ? p->batch - b0 : kBuildMaxBatch;
+            a.ntab = ntab;
+            a.is_double = p->dtype == FRESNEL_C128;
+            a.scal_out = sc >= 0 ? (double *)p->slots[sc].dev : nullptr;
+            for (int b = 0; b < a.nb; ++b) {
+                if (sc >= 0) a.scal[b] = p->slots[sc].key[b0 + b].c_hi;
+                for (int t = 0; t < ntab; ++t) a.t[t].spec[b] = p->slots[chirps[ci + t]].key[b0 + b];
+            }
+            for (int t = 0; t < ntab; ++t) {
+                const TableSlot &s = p->slots[chirps[ci + t]];
+                a.t[t].out = s.dev;
+                a.t[t].index_mode = s.kind;
+                a.t[t].alt_sign = s.alt_sign;
+            }
+            dim3 grid((p->N + 127) / 128, a.nb, ntab > 0 ? ntab : 1);
+            build_tables_kernel<<<grid, 128, 0, p->stream>>>(a);
+            if (cudaGetLastError() != cudaSuccess) return FRESNEL_ERR_CUDA;
+            ++p->launches;
+        }
+        ci += ntab;
+        if (sc >= 0) ++si;
+    }
+    return FRESNEL_OK;
 }
 
 bool valid_positive(const double *v, int n)
@@ -205,7 +291,7 @@ bool valid_positive(const double *v, int n)
     return true;
 }
 
-// ---- TMA tensor map of a wavefront for the column pass ------------------------------------------------
+// ---- TMA tensor maps -------------------------------------------------------------------------------------
 typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
                                   const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
                                   CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
@@ -237,6 +323,16 @@ int query_tma_width(int N, fresnel_dtype dt)
     return 0;
 }
 
+int query_map_box(int N, fresnel_dtype dt)
+{
+    switch (N) {
+#define FR_CASE(NN) case NN: return dt == FRESNEL_C128 ? col_tma_map_box_f64_##NN() : col_tma_map_box_f32_##NN();
+        FR_CASE(64) FR_CASE(128) FR_CASE(256) FR_CASE(512) FR_CASE(1024) FR_CASE(2048) FR_CASE(4096) FR_CASE(8192)
+#undef FR_CASE
+    }
+    return 0;
+}
+
 // The wavefront as a 3-D tensor {2N scalars, N rows, batch}; a box is {2W scalars, 256 rows, 1}.
 bool make_tensor_map(fresnel_plan *p, void *wf)
 {
@@ -261,36 +357,87 @@ bool make_tensor_map(fresnel_plan *p, void *wf)
     return true;
 }
 
+// A real [N][N] surface map as a 2-D tensor {N, N}; a box is {map_box columns, 256 rows} (fused column pass).
+const CUtensorMap *map_tensor_map(fresnel_plan *p, const void *m)
+{
+    ++p->clock;
+    for (MapDesc &d : p->map_descs)
+        if (d.ptr == m) { d.stamp = p->clock; return &d.map; }
+    EncodeTiledFn fn = encode_tiled_fn();
+    if (!fn) return nullptr;
+    MapDesc d;
+    const bool dbl = p->dtype == FRESNEL_C128;
+    const size_t rs = dbl ? sizeof(double) : sizeof(float);
+    const cuuint64_t N = (cuuint64_t)p->N;
+    cuuint64_t gdim[2] = {N, N};
+    cuuint64_t gstr[1] = {N * rs};
+    cuuint32_t box[2] = {(cuuint32_t)p->map_box, 256u};
+    cuuint32_t estr[2] = {1, 1};
+    CUresult r = fn(&d.map, dbl ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<void *>(m), gdim, gstr,
+                    box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return nullptr;
+    d.ptr = m;
+    d.stamp = p->clock;
+    if ((int)p->map_descs.size() < kMaxMapDescs) {
+        p->map_descs.push_back(d);
+        return &p->map_descs.back().map;
+    }
+    size_t victim = 0;
+    for (size_t i = 1; i < p->map_descs.size(); ++i)
+        if (p->map_descs[i].stamp < p->map_descs[victim].stamp) victim = i;
+    p->map_descs[victim] = d;
+    return &p->map_descs[victim].map;
+}
+
 // ---- pass launch by (dtype, N) ---------------------------------------------------------------------
-fresnel_status run_pass(fresnel_plan *p, bool col, int mode, void *wf, const void *pre, const void *rowfac, const void *mid,
-                        const void *amp, const void *opd, double scale)
+// Everything one pass kernel may be asked to do (see pass_kernel.cuh); tables are device pointers of the plan's dtype.
+struct PassSpec {
+    bool col = false;
+    int mode = MODE_CONV;
+    const void *pre = nullptr, *rowfac = nullptr, *mid = nullptr;
+    const void *amp = nullptr, *opd = nullptr;          // load-side optic (row pass only)
+    const void *lens2 = nullptr, *mid2 = nullptr;       // MODE_CONV2
+    const void *amp2 = nullptr, *opd2 = nullptr;
+    const double *inv_lambda = nullptr;
+    double scale = 1.0;
+};
+
+fresnel_status run_pass(fresnel_plan *p, void *wf, const PassSpec &q)
 {
     cudaError_t e = cudaErrorInvalidValue;
-    const bool tma = col && p->tma_w > 0 && make_tensor_map(p, wf);
+    const bool tma = q.col && p->tma_w > 0 && make_tensor_map(p, wf);
+    const CUtensorMap *ma = &p->tmap, *mo = &p->tmap;
+    if (tma && q.mode == MODE_CONV2) {
+        if (q.amp2 && !(ma = map_tensor_map(p, q.amp2))) return FRESNEL_ERR_CUDA;
+        if (q.opd2 && !(mo = map_tensor_map(p, q.opd2))) return FRESNEL_ERR_CUDA;
+    }
     // L2 prefetch of upcoming rows pays when the data does not already sit in the 126 MB L2 (measured:
     // +10..17 % at N >= 4096, -4 % at N = 2048 without maps); TMA tile prefetch of 16..32-byte-wide
     // column boxes costs more TMA issue slots than it saves and stays off.
     const size_t wf_bytes = (size_t)p->batch * p->N * p->N * p->esize();
-    const int prefetch = (!col && (wf_bytes > ((size_t)64 << 20) || amp || opd)) ? p->prefetch : 0;
+    const int prefetch = (!q.col && (wf_bytes > ((size_t)64 << 20) || q.amp || q.opd)) ? p->prefetch : 0;
     if (p->dtype == FRESNEL_C128) {
         PassArgs<double> a;
-        a.wf = (double2 *)wf; a.pre = (const double2 *)pre; a.mid = (const double2 *)mid; a.rowfac = (const double2 *)rowfac;
-        a.tw = (const double2 *)p->tw; a.amp = (const double *)amp; a.opd = (const double *)opd;
-        a.inv_lambda = p->scal_dev; a.scale = scale; a.prefetch_distance = prefetch; a.pdl = p->pdl;
+        a.wf = (double2 *)wf; a.pre = (const double2 *)q.pre; a.mid = (const double2 *)q.mid; a.rowfac = (const double2 *)q.rowfac;
+        a.tw = (const double2 *)p->tw; a.amp = (const double *)q.amp; a.opd = (const double *)q.opd;
+        a.inv_lambda = q.inv_lambda; a.scale = q.scale; a.prefetch_distance = prefetch; a.pdl = p->pdl;
+        a.lens2 = (const double2 *)q.lens2; a.mid2 = (const double2 *)q.mid2; a.amp2 = (const double *)q.amp2; a.opd2 = (const double *)q.opd2;
         switch (p->N) {
-#define FR_CASE(NN) case NN: e = tma ? launch_col_tma_f64_##NN(mode, a, p->tmap, p->batch, p->stream)           \
-                                   : launch_pass_f64_##NN(col, mode, a, p->batch, p->stream); break;
+#define FR_CASE(NN) case NN: e = tma ? launch_col_tma_f64_##NN(q.mode, a, p->tmap, *ma, *mo, p->batch, p->stream)           \
+                                   : launch_pass_f64_##NN(q.col, q.mode, a, p->batch, p->stream); break;
             FR_CASE(64) FR_CASE(128) FR_CASE(256) FR_CASE(512) FR_CASE(1024) FR_CASE(2048) FR_CASE(4096) FR_CASE(8192)
 #undef FR_CASE
         }
     } else {
         PassArgs<float> a;
-        a.wf = (float2 *)wf; a.pre = (const float2 *)pre; a.mid = (const float2 *)mid; a.rowfac = (const float2 *)rowfac;
-        a.tw = (const float2 *)p->tw; a.amp = (const float *)amp; a.opd = (const float *)opd;
-        a.inv_lambda = p->scal_dev; a.scale = (float)scale; a.prefetch_distance = prefetch; a.pdl = p->pdl;
+        a.wf = (float2 *)wf; a.pre = (const float2 *)q.pre; a.mid = (const float2 *)q.mid; a.rowfac = (const float2 *)q.rowfac;
+        a.tw = (const float2 *)p->tw; a.amp = (const float *)q.amp; a.opd = (const float *)q.opd;
+        a.inv_lambda = q.inv_lambda; a.scale = (float)q.scale; a.prefetch_distance = prefetch; a.pdl = p->pdl;
+        a.lens2 = (const float2 *)q.lens2; a.mid2 = (const float2 *)q.mid2; a.amp2 = (const float *)q.amp2; a.opd2 = (const float *)q.opd2;
         switch (p->N) {
-#define FR_CASE(NN) case NN: e = tma ? launch_col_tma_f32_##NN(mode, a, p->tmap, p->batch, p->stream)           \
-                                   : launch_pass_f32_##NN(col, mode, a, p->batch, p->stream); break;
+#define FR_CASE(NN) case NN: e = tma ? launch_col_tma_f32_##NN(q.mode, a, p->tmap, *ma, *mo, p->batch, p->stream)           \
+                                   : launch_pass_f32_##NN(q.col, q.mode, a, p->batch, p->stream); break;
             FR_CASE(64) FR_CASE(128) FR_CASE(256) FR_CASE(512) FR_CASE(1024) FR_CASE(2048) FR_CASE(4096) FR_CASE(8192)
 #undef FR_CASE
         }
@@ -300,33 +447,56 @@ fresnel_status run_pass(fresnel_plan *p, bool col, int mode, void *wf, const voi
     return FRESNEL_OK;
 }
 
+// profiling hook of fresnel_system_run: event k before pass kernel k of the train, one more after the last
+void train_event(fresnel_plan *p, size_t k)
+{
+    if (k < p->train_ev.size()) cudaEventRecord(p->train_ev[k], p->stream);
+}
+
+void note_pass(fresnel_plan *p, int direction, int nconv, int surface, int maps)
+{
+    fresnel_pass_info i;
+    i.direction = direction;
+    i.convolutions = nconv;
+    i.first_surface = surface;
+    i.maps_read = maps;
+    p->schedule.push_back(i);
+}
+
 // The two HBM round trips of a propagation / transform: row pass then column pass.
 fresnel_status run_two_passes(fresnel_plan *p, int mode, void *wf, const void *pre, const void *mid,
-                              const void *amp, const void *opd, double scale)
+                              const void *amp, const void *opd, const double *inv_lambda, double scale, int surface = -1)
 {
     const bool ev = p->ev_armed;
     p->ev_armed = false;
     if (ev && cudaEventRecord(p->ev[0], p->stream) != cudaSuccess) return FRESNEL_ERR_CUDA;
     // the input chirp is separable: its x-part rides on the load of the row pass, its y-part (one factor per
     // row) on the store of the row pass, so the column pass has no input table at all
-    fresnel_status st = run_pass(p, false, mode, wf, pre, pre, mid, amp, opd, scale);
+    PassSpec r;
+    r.col = false; r.mode = mode; r.pre = pre; r.rowfac = pre; r.mid = mid; r.amp = amp; r.opd = opd;
+    r.inv_lambda = inv_lambda; r.scale = scale;
+    if (surface >= 0) { train_event(p, p->schedule.size()); note_pass(p, 0, mode == MODE_CONV ? 1 : 0, surface, (amp != nullptr) + (opd != nullptr)); }
+    fresnel_status st = run_pass(p, wf, r);
     if (st != FRESNEL_OK) return st;
     if (ev && cudaEventRecord(p->ev[1], p->stream) != cudaSuccess) return FRESNEL_ERR_CUDA;
-    st = run_pass(p, true, mode, wf, nullptr, nullptr, mid, nullptr, nullptr, scale);
+    PassSpec c;
+    c.col = true; c.mode = mode; c.mid = mid; c.scale = scale;
+    if (surface >= 0) { train_event(p, p->schedule.size()); note_pass(p, 1, mode == MODE_CONV ? 1 : 0, surface, 0); }
+    st = run_pass(p, wf, c);
     if (st != FRESNEL_OK) return st;
     if (ev && cudaEventRecord(p->ev[2], p->stream) != cudaSuccess) return FRESNEL_ERR_CUDA;
     return FRESNEL_OK;
 }
 
-fresnel_status run_pointwise(fresnel_plan *p, void *wf, const void *tab, const void *amp, const void *opd)
+fresnel_status run_pointwise(fresnel_plan *p, void *wf, const void *tab, const void *amp, const void *opd, const double *inv_lambda)
 {
     cudaError_t e;
     if (p->dtype == FRESNEL_C128)
         e = launch_pointwise<double>((double2 *)wf, (const double2 *)tab, (const double *)amp, (const double *)opd,
-                                     p->scal_dev, p->N, p->batch, p->stream);
+                                     inv_lambda, p->N, p->batch, p->stream);
     else
         e = launch_pointwise<float>((float2 *)wf, (const float2 *)tab, (const float *)amp, (const float *)opd,
-                                    p->scal_dev, p->N, p->batch, p->stream);
+                                    inv_lambda, p->N, p->batch, p->stream);
     if (e != cudaSuccess) return FRESNEL_ERR_CUDA;
     ++p->launches;
     return FRESNEL_OK;
@@ -342,6 +512,139 @@ long double as_coeff(int N, double dx, double lambda, double z)
 {
     long double nd = (long double)N * (long double)dx;
     return -(long double)lambda * (long double)z / (2.0L * nd * nd);
+}
+
+std::vector<ChirpSpec> lens_key(const fresnel_plan *p, const double *pixel, const double *lambda, double f)
+{
+    std::vector<ChirpSpec> key(p->batch);
+    for (int b = 0; b < p->batch; ++b) key[b] = make_spec(qpf_coeff(pixel[b], lambda[b], -(long double)f), 1.0, 0.0);
+    return key;
+}
+std::vector<ChirpSpec> transfer_key(const fresnel_plan *p, const double *pixel, const double *lambda, double z)
+{
+    std::vector<ChirpSpec> key(p->batch);
+    for (int b = 0; b < p->batch; ++b) key[b] = make_spec(as_coeff(p->N, pixel[b], lambda[b], z), 1.0 / (double)p->N, 0.0);
+    return key;
+}
+
+// ---- one fused surface (thin lens + optic phasor + angular spectrum), two passes ------------------------------
+fresnel_status surface_as_impl(fresnel_plan *p, void *wf, const double *pixel, const double *lambda,
+                               double f, const void *amp, const void *opd, double z, int surface = -1)
+{
+    ++p->pin_epoch;
+    const CaptureState cap = capture_state(p);
+    const bool lens = std::isfinite(f);
+    const bool prop = z != 0.0;
+    if (!lens && !prop && !amp && !opd) return FRESNEL_OK;
+
+    TableRequest r[3];
+    int nreq = 0, i_lens = -1, i_h = -1, i_s = -1;
+    if (lens) { i_lens = nreq; r[nreq++] = request_table(p, KIND_CENTRED, 0, lens_key(p, pixel, lambda, f), cap); }
+    if (prop) { i_h = nreq; r[nreq++] = request_table(p, KIND_FFTORDER, 0, transfer_key(p, pixel, lambda, z), cap); }
+    if (opd) { i_s = nreq; r[nreq++] = request_inv_lambda(p, lambda, cap); }
+    fresnel_status st = flush_builds(p, r, nreq);
+    if (st != FRESNEL_OK) return st;
+    const void *tl = lens ? p->slots[r[i_lens].slot].dev : nullptr;
+    const double *il = opd ? (const double *)p->slots[r[i_s].slot].dev : nullptr;
+    if (!prop) {                                                   // optic only
+        if (surface >= 0) { train_event(p, p->schedule.size()); note_pass(p, 0, 0, surface, (amp != nullptr) + (opd != nullptr)); }
+        return run_pointwise(p, wf, tl, amp, opd, il);
+    }
+    const void *th = p->slots[r[i_h].slot].dev;
+    // row pass: optic phasor and x-chirp of the lens on load, FFT, x H1, inverse FFT, y-chirp of the lens (one
+    // factor per row) on store;  column pass: FFT, x H1, inverse FFT
+    return run_two_passes(p, MODE_CONV, wf, tl, th, amp, opd, il, 1.0, surface);
+}
+
+// [thin lens f] -> [optic phasor] -> direct Fresnel propagation by z, in the two passes of the transform:
+// the lens chirp and the input chirp of the propagator are the same kind of factor, so their
+// coefficients are added (long double) and ONE table serves both; the optic phasor rides on the row-pass load.
+fresnel_status direct_impl(fresnel_plan *p, void *wf, double *pixel_inout, const double *lambda, double z,
+                           double f, const void *amp, const void *opd, int surface = -1)
+{
+    ++p->pin_epoch;
+    const CaptureState cap = capture_state(p);
+    const bool lens = std::isfinite(f);
+    std::vector<ChirpSpec> kin(p->batch), kout(p->batch);
+    std::vector<double> dx_out(p->batch);
+    for (int b = 0; b < p->batch; ++b) {
+        const double dx = pixel_inout[b];
+        const long double dxo = (long double)lambda[b] * fabsl((long double)z) / ((long double)p->N * (long double)dx);
+        dx_out[b] = (double)dxo;
+        long double cin = qpf_coeff(dx, lambda[b], z);
+        if (lens) cin += qpf_coeff(dx, lambda[b], -(long double)f);
+        kin[b] = make_spec(cin, 1.0, 0.0);
+        // per-axis share of dx^2/(i lambda z): dx/sqrt(lambda |z|) * exp(-+ i pi/4)
+        const double a1 = (double)((long double)dx / sqrtl((long double)lambda[b] * fabsl((long double)z)));
+        kout[b] = make_spec(qpf_coeff(dx_out[b], lambda[b], z), a1, z > 0 ? -0.125 : 0.125);
+    }
+    // the (-1)^n of the centred transform rides on both tables
+    TableRequest r[3];
+    int nreq = 2;
+    r[0] = request_table(p, KIND_CENTRED, 1, kin, cap);
+    r[1] = request_table(p, KIND_CENTRED, 1, kout, cap);
+    if (opd) r[nreq++] = request_inv_lambda(p, lambda, cap);
+    fresnel_status st = flush_builds(p, r, nreq);
+    if (st != FRESNEL_OK) return st;
+    const double *il = opd ? (const double *)p->slots[r[2].slot].dev : nullptr;
+    const int mode = z > 0 ? MODE_FWD : MODE_INV;
+    st = run_two_passes(p, mode, wf, p->slots[r[0].slot].dev, p->slots[r[1].slot].dev, amp, opd, il, 1.0, surface);
+    if (st != FRESNEL_OK) return st;
+    for (int b = 0; b < p->batch; ++b) pixel_inout[b] = dx_out[b];
+    return FRESNEL_OK;
+}
+
+// ---- a run of consecutive angular-spectrum surfaces, fused at train level ---------------------------------------
+// Surfaces s0 .. s0+L-1 (all with z != 0, same pixel pitch).  Row and column convolution of a surface commute, so the
+// passes are ordered
+//     rows_0 (with optic_0 on load) | cols_0, optic_1, cols_1 | rows_1, optic_2, rows_2 | ... | last convolution
+// i.e. L+1 kernels instead of 2L: kernel k (1 <= k < L) runs along columns for odd k and along rows for even k and
+// holds every line resident through  conv_{k-1} -> optic_k -> conv_k  (MODE_CONV2).
+fresnel_status fused_chain(fresnel_plan *p, void *wf, const double *pixel, const double *lambda,
+                           const fresnel_surface *surf, int s0, int L)
+{
+    ++p->pin_epoch;
+    const CaptureState cap = capture_state(p);
+    std::vector<TableRequest> req;
+    std::vector<int> i_lens(L, -1), i_h(L, -1);
+    int i_s = -1;
+    bool any_opd = false;
+    for (int k = 0; k < L; ++k) {
+        const fresnel_surface &q = surf[s0 + k];
+        if (std::isfinite(q.f)) { i_lens[k] = (int)req.size(); req.push_back(request_table(p, KIND_CENTRED, 0, lens_key(p, pixel, lambda, q.f), cap)); }
+        i_h[k] = (int)req.size();
+        req.push_back(request_table(p, KIND_FFTORDER, 0, transfer_key(p, pixel, lambda, q.z), cap));
+        any_opd = any_opd || q.opd != nullptr;
+    }
+    if (any_opd) { i_s = (int)req.size(); req.push_back(request_inv_lambda(p, lambda, cap)); }
+    fresnel_status st = flush_builds(p, req.data(), (int)req.size());
+    if (st != FRESNEL_OK) return st;
+    auto lens = [&](int k) -> const void * { return i_lens[k] >= 0 ? p->slots[req[i_lens[k]].slot].dev : nullptr; };
+    auto H = [&](int k) -> const void * { return p->slots[req[i_h[k]].slot].dev; };
+    const double *il = any_opd ? (const double *)p->slots[req[i_s].slot].dev : nullptr;
+
+    for (int k = 0; k <= L; ++k) {
+        PassSpec q;
+        q.col = (k & 1) != 0;
+        q.inv_lambda = il;
+        int maps = 0;
+        if (k == 0) {                       // optic_0 on load, rows_0
+            const fresnel_surface &s = surf[s0];
+            q.mode = MODE_CONV; q.pre = lens(0); q.rowfac = lens(0); q.mid = H(0); q.amp = s.amp; q.opd = s.opd;
+            maps = (s.amp != nullptr) + (s.opd != nullptr);
+        } else if (k < L) {                 // conv_{k-1}, optic_k, conv_k along the same direction
+            const fresnel_surface &s = surf[s0 + k];
+            q.mode = MODE_CONV2; q.mid = H(k - 1); q.lens2 = lens(k); q.amp2 = s.amp; q.opd2 = s.opd; q.mid2 = H(k);
+            maps = (s.amp != nullptr) + (s.opd != nullptr);
+        } else {                            // the remaining convolution of the last surface
+            q.mode = MODE_CONV; q.mid = H(L - 1);
+        }
+        train_event(p, p->schedule.size());
+        note_pass(p, q.col ? 1 : 0, (k > 0 && k < L) ? 2 : 1, s0 + (k < L ? k : L - 1), maps);
+        st = run_pass(p, wf, q);
+        if (st != FRESNEL_OK) return st;
+    }
+    return FRESNEL_OK;
 }
 
 } // namespace
@@ -361,7 +664,7 @@ const char *fresnel_status_string(fresnel_status s)
     return "FRESNEL_ERR_UNKNOWN";
 }
 
-const char *fresnel_version(void) { return "fresnel-b200 0.1 sm_100a"; }
+const char *fresnel_version(void) { return "fresnel-b200 0.2 sm_100a"; }
 
 fresnel_status fresnel_plan_create(fresnel_plan **out, int N, int batch, fresnel_dtype dtype)
 {
@@ -375,45 +678,83 @@ fresnel_status fresnel_plan_create(fresnel_plan **out, int N, int batch, fresnel
     p->N = N; p->batch = batch; p->dtype = dtype;
     {
         int sms = 148;
-        int dev = 0;
-        cudaGetDevice(&dev);
-        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        cudaGetDevice(&p->device);
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, p->device);
         p->sms = sms;
         const char *pf = std::getenv("FRESNEL_PREFETCH");          // tuning only: tiles ahead, 0 = off
         p->prefetch = pf ? std::atoi(pf) : -sms;                   // negative: auto = SMs x resident CTAs per SM
     }
     { const char *pd = std::getenv("FRESNEL_PDL"); p->pdl = pd ? std::atoi(pd) : 1; }
+    { const char *fu = std::getenv("FRESNEL_FUSE"); p->fuse = fu ? std::atoi(fu) : 1; }
     p->tma_w = std::getenv("FRESNEL_NO_TMA") ? 0 : query_tma_width(N, dtype);     // env switch: A/B timing only
+    p->map_box = query_map_box(N, dtype);
+    p->map_descs.reserve(kMaxMapDescs);                            // pointers into it are handed out
     fresnel_status st = upload_twiddles(p);
-    if (st == FRESNEL_OK && cudaMalloc((void **)&p->scal_dev, sizeof(double) * batch) != cudaSuccess) st = FRESNEL_ERR_ALLOC;
-    for (int i = 0; i < kSlots && st == FRESNEL_OK; ++i)
-        if (cudaMalloc(&p->slots[i].dev, (size_t)batch * N * p->esize()) != cudaSuccess) st = FRESNEL_ERR_ALLOC;
+    if (st == FRESNEL_OK && cudaEventCreateWithFlags(&p->order_ev, cudaEventDisableTiming) != cudaSuccess) st = FRESNEL_ERR_CUDA;
+    if (st == FRESNEL_OK) st = grow_slots(p, kDefaultSlots);
     if (st != FRESNEL_OK) { cudaGetLastError(); fresnel_plan_destroy(p); return st; }
     *out = p;
+    return FRESNEL_OK;
+}
+
+fresnel_status fresnel_plan_reserve_tables(fresnel_plan *p, int n_tables)
+{
+    if (!p || n_tables < 0) return FRESNEL_ERR_INVALID_ARG;
+    DeviceGuard g(p);
+    if (capture_state(p).active) return FRESNEL_ERR_UNSUPPORTED;  // allocates: not while capturing
+    return grow_slots(p, n_tables - eager_slot_count(p));
+}
+
+fresnel_status fresnel_plan_release_graph_tables(fresnel_plan *p)
+{
+    if (!p) return FRESNEL_ERR_INVALID_ARG;
+    for (TableSlot &s : p->slots)
+        if (s.graph_owned) { s.graph_owned = false; s.valid = false; s.capture_id = 0; }
     return FRESNEL_OK;
 }
 
 fresnel_status fresnel_plan_set_stream(fresnel_plan *p, void *cuda_stream)
 {
     if (!p) return FRESNEL_ERR_INVALID_ARG;
-    p->stream = (cudaStream_t)cuda_stream;
+    DeviceGuard g(p);
+    cudaStream_t ns = (cudaStream_t)cuda_stream;
+    if (ns == p->stream) return FRESNEL_OK;
+    // Tables built (and kernels reading them) on the old stream must precede whatever the new stream does with the
+    // same slots: the new stream waits for the old one's tail.  Not possible across a capture boundary.
+    cudaStreamCaptureStatus so = cudaStreamCaptureStatusNone, sn = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(p->stream, &so) != cudaSuccess) { cudaGetLastError(); so = cudaStreamCaptureStatusNone; }
+    if (cudaStreamIsCapturing(ns, &sn) != cudaSuccess) { cudaGetLastError(); sn = cudaStreamCaptureStatusNone; }
+    if (so == cudaStreamCaptureStatusNone && sn == cudaStreamCaptureStatusNone) {
+        if (cudaEventRecord(p->order_ev, p->stream) != cudaSuccess || cudaStreamWaitEvent(ns, p->order_ev, 0) != cudaSuccess) {
+            cudaGetLastError();
+            return FRESNEL_ERR_CUDA;
+        }
+    } else {
+        for (TableSlot &s : p->slots)                              // cannot be ordered: forget the eager tables
+            if (!s.graph_owned) s.valid = false;
+    }
+    p->stream = ns;
     return FRESNEL_OK;
 }
 
 fresnel_status fresnel_plan_synchronize(fresnel_plan *p)
 {
     if (!p) return FRESNEL_ERR_INVALID_ARG;
+    DeviceGuard g(p);
     return cudaStreamSynchronize(p->stream) == cudaSuccess ? FRESNEL_OK : FRESNEL_ERR_CUDA;
 }
 
 fresnel_status fresnel_plan_destroy(fresnel_plan *p)
 {
     if (!p) return FRESNEL_OK;
-    cudaStreamSynchronize(p->stream);
-    cudaFree(p->tw);
-    cudaFree(p->scal_dev);
-    for (int i = 0; i < kSlots; ++i) cudaFree(p->slots[i].dev);
-    cudaGetLastError();
+    {
+        DeviceGuard g(p);
+        cudaStreamSynchronize(p->stream);
+        cudaFree(p->tw);
+        for (void *a : p->arenas) cudaFree(a);
+        if (p->order_ev) cudaEventDestroy(p->order_ev);
+        cudaGetLastError();
+    }
     delete p;
     return FRESNEL_OK;
 }
@@ -437,15 +778,36 @@ fresnel_status fresnel_plan_record_pass_events(fresnel_plan *p, void *const even
     return FRESNEL_OK;
 }
 
+fresnel_status fresnel_plan_record_train_events(fresnel_plan *p, void *const *events, int n_events)
+{
+    if (!p || n_events < 0 || (n_events > 0 && !events)) return FRESNEL_ERR_INVALID_ARG;
+    p->train_ev.clear();
+    for (int i = 0; i < n_events; ++i) {
+        if (!events[i]) { p->train_ev.clear(); return FRESNEL_ERR_INVALID_ARG; }
+        p->train_ev.push_back((cudaEvent_t)events[i]);
+    }
+    return FRESNEL_OK;
+}
+
+fresnel_status fresnel_plan_last_schedule(const fresnel_plan *p, fresnel_pass_info *out, int capacity, int *count)
+{
+    if (!p || !count || capacity < 0 || (capacity > 0 && !out)) return FRESNEL_ERR_INVALID_ARG;
+    *count = (int)p->schedule.size();
+    for (int i = 0; i < capacity && i < *count; ++i) out[i] = p->schedule[i];
+    return FRESNEL_OK;
+}
+
 fresnel_status fresnel_memcpy_h2d(fresnel_plan *p, void *dst_device, const void *src_host, size_t bytes)
 {
     if (!p || !dst_device || !src_host) return FRESNEL_ERR_INVALID_ARG;
+    DeviceGuard g(p);
     return cudaMemcpyAsync(dst_device, src_host, bytes, cudaMemcpyHostToDevice, p->stream) == cudaSuccess ? FRESNEL_OK : FRESNEL_ERR_CUDA;
 }
 
 fresnel_status fresnel_memcpy_d2h(fresnel_plan *p, void *dst_host, const void *src_device, size_t bytes)
 {
     if (!p || !dst_host || !src_device) return FRESNEL_ERR_INVALID_ARG;
+    DeviceGuard g(p);
     return cudaMemcpyAsync(dst_host, src_device, bytes, cudaMemcpyDeviceToHost, p->stream) == cudaSuccess ? FRESNEL_OK : FRESNEL_ERR_CUDA;
 }
 
@@ -454,14 +816,15 @@ fresnel_status fresnel_apply_qpf(fresnel_plan *p, void *wf, const double *pixel,
 {
     if (!p || !wf || !valid_positive(pixel, p ? p->batch : 0) || !valid_positive(lambda, p->batch)) return FRESNEL_ERR_INVALID_ARG;
     if (!std::isfinite(z) || z == 0.0) return FRESNEL_ERR_INVALID_ARG;
-    ++p->call_id;
-    const bool force = capturing(p);
+    DeviceGuard g(p);
+    ++p->pin_epoch;
+    const CaptureState cap = capture_state(p);
     std::vector<ChirpSpec> key(p->batch);
     for (int b = 0; b < p->batch; ++b) key[b] = make_spec(qpf_coeff(pixel[b], lambda[b], z), 1.0, 0.0);
-    TableRequest r = request_table(p, 0, 0, key, force);
-    fresnel_status st = flush_builds(p, &r, 1, nullptr);
+    TableRequest r = request_table(p, KIND_CENTRED, 0, key, cap);
+    fresnel_status st = flush_builds(p, &r, 1);
     if (st != FRESNEL_OK) return st;
-    return run_pointwise(p, wf, p->slots[r.slot].dev, nullptr, nullptr);
+    return run_pointwise(p, wf, p->slots[r.slot].dev, nullptr, nullptr, nullptr);
 }
 
 // ---- Eq. 3: optic phasor ------------------------------------------------------------------------------
@@ -469,32 +832,38 @@ fresnel_status fresnel_apply_mask(fresnel_plan *p, void *wf, const void *amp, co
 {
     if (!p || !wf || !valid_positive(lambda, p ? p->batch : 0)) return FRESNEL_ERR_INVALID_ARG;
     if (!amp && !opd) return FRESNEL_OK;
-    ++p->call_id;
-    std::vector<double> tmp;
-    const double *scal = opd ? need_inv_lambda(p, lambda, tmp, capturing(p)) : nullptr;
-    fresnel_status st = flush_builds(p, nullptr, 0, scal);
-    if (st != FRESNEL_OK) return st;
-    return run_pointwise(p, wf, nullptr, amp, opd);
+    DeviceGuard g(p);
+    ++p->pin_epoch;
+    const double *il = nullptr;
+    if (opd) {
+        TableRequest r = request_inv_lambda(p, lambda, capture_state(p));
+        fresnel_status st = flush_builds(p, &r, 1);
+        if (st != FRESNEL_OK) return st;
+        il = (const double *)p->slots[r.slot].dev;
+    }
+    return run_pointwise(p, wf, nullptr, amp, opd, il);
 }
 
 // ---- 2-D FFT ---------------------------------------------------------------------------------------------
 fresnel_status fresnel_fft2d(fresnel_plan *p, void *wf, int direction, int centered)
 {
     if (!p || !wf || (direction != FRESNEL_FORWARD && direction != FRESNEL_INVERSE)) return FRESNEL_ERR_INVALID_ARG;
-    ++p->call_id;
+    DeviceGuard g(p);
+    ++p->pin_epoch;
     const int mode = direction == FRESNEL_FORWARD ? MODE_FWD : MODE_INV;
     const double per_pass = direction == FRESNEL_FORWARD ? 1.0 : 1.0 / (double)p->N;
     if (!centered) {
-        return run_two_passes(p, mode, wf, nullptr, nullptr, nullptr, nullptr, per_pass);
+        return run_two_passes(p, mode, wf, nullptr, nullptr, nullptr, nullptr, nullptr, per_pass);
     }
     // centred transform = s * fft2(s * u), s = (-1)^(j+k): sign tables on load and after the transform
-    const bool force = capturing(p);
+    const CaptureState cap = capture_state(p);
     std::vector<ChirpSpec> k1(p->batch, make_spec(0.0L, 1.0, 0.0)), k2(p->batch, make_spec(0.0L, per_pass, 0.0));
-    TableRequest r[2] = {request_table(p, 0, 1, k1, force), request_table(p, 0, 1, k2, force)};
-    if (r[0].slot == r[1].slot) r[1].build = false;
-    fresnel_status st = flush_builds(p, r, 2, nullptr);
+    TableRequest r[2];
+    r[0] = request_table(p, KIND_CENTRED, 1, k1, cap);
+    r[1] = request_table(p, KIND_CENTRED, 1, k2, cap);
+    fresnel_status st = flush_builds(p, r, 2);
     if (st != FRESNEL_OK) return st;
-    return run_two_passes(p, mode, wf, p->slots[r[0].slot].dev, p->slots[r[1].slot].dev, nullptr, nullptr, 1.0);
+    return run_two_passes(p, mode, wf, p->slots[r[0].slot].dev, p->slots[r[1].slot].dev, nullptr, nullptr, nullptr, 1.0);
 }
 
 // ---- fused surface: lens + optic phasor + angular-spectrum propagation ----------------------------
@@ -503,35 +872,8 @@ fresnel_status fresnel_surface_as(fresnel_plan *p, void *wf, const double *pixel
 {
     if (!p || !wf || !valid_positive(pixel, p ? p->batch : 0) || !valid_positive(lambda, p->batch)) return FRESNEL_ERR_INVALID_ARG;
     if (!std::isfinite(z) || std::isnan(f) || f == 0.0) return FRESNEL_ERR_INVALID_ARG;
-    ++p->call_id;
-    const bool force = capturing(p);
-    const bool lens = std::isfinite(f);
-    const bool prop = z != 0.0;
-    if (!lens && !prop && !amp && !opd) return FRESNEL_OK;
-
-    TableRequest r[2];
-    int nreq = 0, i_lens = -1, i_h = -1;
-    std::vector<ChirpSpec> key(p->batch);
-    if (lens) {
-        for (int b = 0; b < p->batch; ++b) key[b] = make_spec(qpf_coeff(pixel[b], lambda[b], -(long double)f), 1.0, 0.0);
-        i_lens = nreq;
-        r[nreq++] = request_table(p, 0, 0, key, force);
-    }
-    if (prop) {
-        for (int b = 0; b < p->batch; ++b) key[b] = make_spec(as_coeff(p->N, pixel[b], lambda[b], z), 1.0 / (double)p->N, 0.0);
-        i_h = nreq;
-        r[nreq++] = request_table(p, 1, 0, key, force);
-    }
-    std::vector<double> tmp;
-    const double *scal = opd ? need_inv_lambda(p, lambda, tmp, force) : nullptr;
-    fresnel_status st = flush_builds(p, r, nreq, scal);
-    if (st != FRESNEL_OK) return st;
-    const void *tl = lens ? p->slots[r[i_lens].slot].dev : nullptr;
-    if (!prop) return run_pointwise(p, wf, tl, amp, opd);          // optic only
-    const void *th = p->slots[r[i_h].slot].dev;
-    // row pass: optic phasor and x-chirp of the lens on load, FFT, x H1, inverse FFT, y-chirp of the lens (one
-    // factor per row) on store;  column pass: FFT, x H1, inverse FFT
-    return run_two_passes(p, MODE_CONV, wf, tl, th, amp, opd, 1.0);
+    DeviceGuard g(p);
+    return surface_as_impl(p, wf, pixel, lambda, f, amp, opd, z);
 }
 
 fresnel_status fresnel_propagate_as(fresnel_plan *p, void *wf, const double *pixel, const double *lambda, double z)
@@ -540,53 +882,11 @@ fresnel_status fresnel_propagate_as(fresnel_plan *p, void *wf, const double *pix
 }
 
 // ---- direct (single-FFT) Fresnel ---------------------------------------------------------------------
-} // extern "C"
-
-namespace {
-
-// [thin lens f] -> [optic phasor] -> direct Fresnel propagation by z, in the two passes of the transform:
-// the lens chirp and the input chirp of the propagator are the same kind of factor, so their
-// coefficients are added (long double) and ONE table serves both; the optic phasor rides on the row-pass load.
-fresnel_status direct_impl(fresnel_plan *p, void *wf, double *pixel_inout, const double *lambda, double z,
-                           double f, const void *amp, const void *opd)
-{
-    ++p->call_id;
-    const bool force = capturing(p);
-    const bool lens = std::isfinite(f);
-    std::vector<ChirpSpec> kin(p->batch), kout(p->batch);
-    std::vector<double> dx_out(p->batch);
-    for (int b = 0; b < p->batch; ++b) {
-        const double dx = pixel_inout[b];
-        const long double dxo = (long double)lambda[b] * fabsl((long double)z) / ((long double)p->N * (long double)dx);
-        dx_out[b] = (double)dxo;
-        long double cin = qpf_coeff(dx, lambda[b], z);
-        if (lens) cin += qpf_coeff(dx, lambda[b], -(long double)f);
-        kin[b] = make_spec(cin, 1.0, 0.0);
-        // per-axis share of dx^2/(i lambda z): dx/sqrt(lambda |z|) * exp(-+ i pi/4)
-        const double a1 = (double)((long double)dx / sqrtl((long double)lambda[b] * fabsl((long double)z)));
-        kout[b] = make_spec(qpf_coeff(dx_out[b], lambda[b], z), a1, z > 0 ? -0.125 : 0.125);
-    }
-    // the (-1)^n of the centred transform rides on both tables
-    TableRequest r[2] = {request_table(p, 0, 1, kin, force), request_table(p, 0, 1, kout, force)};
-    std::vector<double> tmp;
-    const double *scal = opd ? need_inv_lambda(p, lambda, tmp, force) : nullptr;
-    fresnel_status st = flush_builds(p, r, 2, scal);
-    if (st != FRESNEL_OK) return st;
-    const int mode = z > 0 ? MODE_FWD : MODE_INV;
-    st = run_two_passes(p, mode, wf, p->slots[r[0].slot].dev, p->slots[r[1].slot].dev, amp, opd, 1.0);
-    if (st != FRESNEL_OK) return st;
-    for (int b = 0; b < p->batch; ++b) pixel_inout[b] = dx_out[b];
-    return FRESNEL_OK;
-}
-
-} // namespace
-
-extern "C" {
-
 fresnel_status fresnel_propagate_direct(fresnel_plan *p, void *wf, double *pixel_inout, const double *lambda, double z)
 {
     if (!p || !wf || !valid_positive(pixel_inout, p ? p->batch : 0) || !valid_positive(lambda, p->batch)) return FRESNEL_ERR_INVALID_ARG;
     if (!std::isfinite(z) || z == 0.0) return FRESNEL_ERR_INVALID_ARG;
+    DeviceGuard g(p);
     return direct_impl(p, wf, pixel_inout, lambda, z, INFINITY, nullptr, nullptr);
 }
 
@@ -596,6 +896,7 @@ fresnel_status fresnel_system_run(fresnel_plan *p, void *wf, double *pixel_inout
 {
     if (!p || !wf || nsurf < 0 || (nsurf > 0 && !surf)) return FRESNEL_ERR_INVALID_ARG;
     if (!valid_positive(pixel_inout, p->batch) || !valid_positive(lambda, p->batch)) return FRESNEL_ERR_INVALID_ARG;
+    DeviceGuard g(p);
     // dry run on the host: validate everything and fix the propagator of every surface before anything is enqueued
     std::vector<int> method(nsurf);
     std::vector<long double> dx(p->batch);
@@ -623,15 +924,37 @@ fresnel_status fresnel_system_run(fresnel_plan *p, void *wf, double *pixel_inout
                 if (!(dx[b] > 0.0L) || !std::isfinite((double)dx[b])) return FRESNEL_ERR_INVALID_ARG;
             }
     }
-    for (int s = 0; s < nsurf; ++s) {
-        const fresnel_surface &q = surf[s];
+    p->schedule.clear();
+    auto finish = [&](fresnel_status st) {
+        if (st == FRESNEL_OK) train_event(p, p->schedule.size());
+        p->train_ev.clear();
+        return st;
+    };
+    // a fused run needs all its tables at once (two per surface + 1/lambda): bounded by the eager slots at hand
+    const int avail = eager_slot_count(p);
+    const int max_run = (avail - 4) / 2;
+    int s = 0;
+    while (s < nsurf) {
         fresnel_status st;
-        if (method[s] == FRESNEL_METHOD_DIRECT) st = direct_impl(p, wf, pixel_inout, lambda, q.z, q.f, q.amp, q.opd);
-        else st = fresnel_surface_as(p, wf, pixel_inout, lambda, q.f, q.amp, q.opd, q.z);   // z == 0: optic only
-        if (st != FRESNEL_OK) return st;
+        int L = 0;
+        if (p->fuse && max_run >= 2)
+            while (s + L < nsurf && L < max_run && method[s + L] == FRESNEL_METHOD_AS) ++L;
+        if (L >= 2) {
+            st = fused_chain(p, wf, pixel_inout, lambda, surf, s, L);
+            if (st != FRESNEL_OK) return finish(st);
+            if (method_used)
+                for (int k = 0; k < L; ++k) method_used[s + k] = FRESNEL_METHOD_AS;
+            s += L;
+            continue;
+        }
+        const fresnel_surface &q = surf[s];
+        if (method[s] == FRESNEL_METHOD_DIRECT) st = direct_impl(p, wf, pixel_inout, lambda, q.z, q.f, q.amp, q.opd, s);
+        else st = surface_as_impl(p, wf, pixel_inout, lambda, q.f, q.amp, q.opd, q.z, s);   // z == 0: optic only
+        if (st != FRESNEL_OK) return finish(st);
         if (method_used) method_used[s] = method[s];
+        ++s;
     }
-    return FRESNEL_OK;
+    return finish(FRESNEL_OK);
 }
 
 // ---- broadband image: incoherent sum over the batch ---------------------------------------------------------
@@ -640,6 +963,7 @@ fresnel_status fresnel_accumulate_intensity(fresnel_plan *p, const void *wf, con
     if (!p || !wf || !weight || !image) return FRESNEL_ERR_INVALID_ARG;
     for (int b = 0; b < p->batch; ++b)
         if (!std::isfinite(weight[b])) return FRESNEL_ERR_INVALID_ARG;
+    DeviceGuard g(p);
     cudaError_t e;
     if (p->dtype == FRESNEL_C128)
         e = launch_intensity<double>((const double2 *)wf, (double *)image, weight, p->N, p->batch, p->sms, p->stream, &p->launches);

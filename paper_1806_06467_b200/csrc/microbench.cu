@@ -4,9 +4,10 @@
 //   MEASURED_PEAKS.json does not carry; and the IN-SM rates of the transform itself (no HBM): the stage code
 //   of fft_core.cuh on registers + shared memory only -- butterflies alone, exchanges alone, both -- in SM
 //   cycles per element, next to a synthetic stream that interleaves DFMA with 128-bit shared-memory traffic
-//   in every warp (what the two pipes can do when nothing orders them), and warp shuffles mixed with shared-memory
-//   traffic (they share one pipe), and register <-> tensor-memory moves (tcgen05.st/ld) beside shared-memory traffic
-//   (a separate, faster path).   Build + run:
+//   in every warp (what the two pipes can do when nothing orders them).  These are the numbers bench.py's
+//   `roofline.alu.peak_tflops` and DESIGN.md's "balance" paragraph quote (profiles/r01_microbench.txt; the
+//   shuffle / tensor-memory lines of that file came from probes that are no longer part of the repository).
+//   Build + run:
 //     python -m paper_1806_06467_b200.build --microbench && ./paper_1806_06467_b200/microbench
 #include <cstdio>
 #include <cstdlib>
@@ -230,157 +231,6 @@ template <int NM, int NX, int WARPS> void run_overlap(double clock_hz){
   cudaFree(out);
 }
 
-// do warp shuffles have a data path of their own?  NS shfl.sync (32-bit) and/or NX (STS.128 + LDS.128) pairs per warp-iteration
-template <int NS, int NX, int WARPS>
-__global__ void __launch_bounds__(WARPS * 32, 1) shflmix(int iters, float* out){
-  extern __shared__ double2 sm3[];
-  const int tid = threadIdx.x, lane = tid & 31;
-  float s[8];
-  #pragma unroll
-  for (int i = 0; i < 8; ++i) s[i] = tid + i;
-  double2 v[8];
-  #pragma unroll
-  for (int i = 0; i < 8; ++i) v[i] = make_double2(tid, i);
-  const unsigned base = (unsigned)__cvta_generic_to_shared(sm3 + tid);
-  for (int it = 0; it < iters; ++it) {
-    #pragma unroll
-    for (int u = 0; u < (NS / 8 > NX ? NS / 8 : NX); ++u) {
-      if (u < NX) asm volatile("st.shared.v2.f64 [%0], {%1, %2};" ::"r"(base + (u & 7) * WARPS * 32 * 16), "d"(v[u & 7].x), "d"(v[u & 7].y) : "memory");
-      if (u < NS / 8) {
-        #pragma unroll
-        for (int i = 0; i < 8; ++i) s[i] = __shfl_sync(0xffffffffu, s[i], (lane + 1 + i) & 31) + 1.0f;
-      }
-      if (u < NX) asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v[(u + 3) & 7].x), "=d"(v[(u + 3) & 7].y) : "r"(base + ((u + 5) & 7) * WARPS * 32 * 16) : "memory");
-    }
-  }
-  float r = 0;
-  #pragma unroll
-  for (int i = 0; i < 8; ++i) r += s[i] + (float)v[i].x + (float)v[i].y;
-  out[blockIdx.x * WARPS * 32 + tid] = r;
-}
-template <int NS, int NX, int WARPS> void run_shfl(double clock_hz){
-  float* out; CK(cudaMalloc(&out, 148 * 1024 * 4));
-  const int smem = WARPS * 32 * 8 * 16;
-  CK(cudaFuncSetAttribute(shflmix<NS, NX, WARPS>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-  const int iters = 4000;
-  float ms = timeit([&]{ shflmix<NS, NX, WARPS><<<148, WARPS * 32, smem>>>(iters, out); }, 3);
-  CK(cudaGetLastError());
-  printf("  shuffle warps/SM=%2d shfl=%3d lds+sts=%2d per warp-iteration: %7.1f clk   (shared-memory pipe alone %4.0f, shfl at 1 warp-instr/clk/SM %4.0f)\n",
-         WARPS, NS, NX * 2, ms * 1e-3 * clock_hz / iters, WARPS * NX * 2 * 4.0, (double)WARPS * NS);
-  cudaFree(out);
-}
-
-// tensor memory as an exchange path: NT (tcgen05.st + tcgen05.ld, 32x32b.x16) pairs and/or NX (STS.128 + LDS.128)
-// pairs per warp-iteration, 16 warps per SM
-template <int NT, int NX>
-__global__ void __launch_bounds__(512, 1) tmemmix(int iters, float* out){
-  extern __shared__ double2 sm4[];
-  __shared__ unsigned tbase;
-  const int tid = threadIdx.x, warp = tid / 32;
-  if (warp == 0) {
-    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(&tbase)), "r"(512u) : "memory");
-    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
-  }
-  __syncthreads();
-  asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-  const unsigned taddr = tbase + (((unsigned)(warp & 3) * 32u) << 16) + (unsigned)(warp / 4) * 64u;   // lane quarter of this warp, own columns
-  unsigned r[16];
-  #pragma unroll
-  for (int i = 0; i < 16; ++i) r[i] = tid * 16 + i;
-  double2 v[8];
-  #pragma unroll
-  for (int i = 0; i < 8; ++i) v[i] = make_double2(tid, i);
-  const unsigned base = (unsigned)__cvta_generic_to_shared(sm4 + tid);
-  for (int it = 0; it < iters; ++it) {
-    #pragma unroll
-    for (int u = 0; u < (NT > NX ? NT : NX); ++u) {
-      if (u < NX) asm volatile("st.shared.v2.f64 [%0], {%1, %2};" ::"r"(base + (u & 7) * 512 * 16), "d"(v[u & 7].x), "d"(v[u & 7].y) : "memory");
-      if (u < NT) {
-        asm volatile("tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16};"
-                     ::"r"(taddr + (u & 3) * 16), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]),
-                       "r"(r[8]), "r"(r[9]), "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15]) : "memory");
-        asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
-        asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
-                     : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
-                       "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
-                     : "r"(taddr + ((u + 1) & 3) * 16) : "memory");
-        asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-      }
-      if (u < NX) asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v[(u + 3) & 7].x), "=d"(v[(u + 3) & 7].y) : "r"(base + ((u + 5) & 7) * 512 * 16) : "memory");
-    }
-  }
-  float s = 0;
-  #pragma unroll
-  for (int i = 0; i < 16; ++i) s += (float)r[i];
-  #pragma unroll
-  for (int i = 0; i < 8; ++i) s += (float)v[i].x + (float)v[i].y;
-  out[blockIdx.x * 512 + tid] = s;
-  __syncthreads();
-  if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tbase), "r"(512u) : "memory");
-}
-template <int NT, int NX> void run_tmem(double clock_hz){
-  float* out; CK(cudaMalloc(&out, 148 * 512 * 4));
-  const int smem = 512 * 8 * 16;
-  CK(cudaFuncSetAttribute(tmemmix<NT, NX>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-  const int iters = 2000;
-  float ms = timeit([&]{ tmemmix<NT, NX><<<148, 512, smem>>>(iters, out); }, 3);
-  CK(cudaGetLastError());
-  const double clk = ms * 1e-3 * clock_hz / iters;
-  printf("  tmem warps/SM=16 (tcgen05.st+ld x16) pairs=%d (lds+sts.128) pairs=%d per warp-iteration: %7.1f clk  -> tensor memory %4.0f B/clk/SM  (shared-memory pipe alone %4d clk)\n",
-         NT, NX, clk, NT ? 16.0 * NT * 4096 / clk : 0.0, 16 * NX * 2 * 4);
-  cudaFree(out);
-}
-
-// which (lane, column) of tensor memory lands in which thread / register for the non-trivial tcgen05.ld shapes:
-// one warp writes value (lane << 16 | column) with 32x32b.x16 (thread = lane, register = column), reads it back with
-// 16x64b.x2, 16x128b.x2 and 16x256b.x1, and the host checks the formulas printed below
-__global__ void tmemprobe(unsigned* out){
-  __shared__ unsigned tbase;
-  const int t = threadIdx.x;
-  asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(&tbase)), "r"(32u) : "memory");
-  asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
-  __syncwarp();
-  asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-  const unsigned ta = tbase;
-  unsigned w[16];
-  for (int c = 0; c < 16; ++c) w[c] = (t << 16) | c;
-  asm volatile("tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16};"
-               ::"r"(ta), "r"(w[0]), "r"(w[1]), "r"(w[2]), "r"(w[3]), "r"(w[4]), "r"(w[5]), "r"(w[6]), "r"(w[7]),
-                 "r"(w[8]), "r"(w[9]), "r"(w[10]), "r"(w[11]), "r"(w[12]), "r"(w[13]), "r"(w[14]), "r"(w[15]) : "memory");
-  asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
-  unsigned a[2], b[4], c[4];
-  asm volatile("tcgen05.ld.sync.aligned.16x64b.x2.b32 {%0, %1}, [%2];" : "=r"(a[0]), "=r"(a[1]) : "r"(ta) : "memory");
-  asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-  asm volatile("tcgen05.ld.sync.aligned.16x128b.x2.b32 {%0, %1, %2, %3}, [%4];" : "=r"(b[0]), "=r"(b[1]), "=r"(b[2]), "=r"(b[3]) : "r"(ta) : "memory");
-  asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-  asm volatile("tcgen05.ld.sync.aligned.16x256b.x1.b32 {%0, %1, %2, %3}, [%4];" : "=r"(c[0]), "=r"(c[1]), "=r"(c[2]), "=r"(c[3]) : "r"(ta) : "memory");
-  asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-  for (int i = 0; i < 2; ++i) out[t * 16 + i] = a[i];
-  for (int i = 0; i < 4; ++i) out[t * 16 + 4 + i] = b[i];
-  for (int i = 0; i < 4; ++i) out[t * 16 + 8 + i] = c[i];
-  __syncwarp();
-  asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tbase), "r"(32u) : "memory");
-}
-void run_tmemprobe(){
-  unsigned *d, h[32 * 16];
-  CK(cudaMalloc(&d, sizeof(h))); CK(cudaMemset(d, 0xff, sizeof(h)));
-  tmemprobe<<<1, 32>>>(d);
-  CK(cudaDeviceSynchronize());
-  CK(cudaMemcpy(h, d, sizeof(h), cudaMemcpyDeviceToHost));
-  bool ok64 = true, ok128 = true, ok256 = true;
-  for (int t = 0; t < 32; ++t) {
-    const int a = t / 4, c = t % 4;
-    for (int k = 0; k < 2; ++k) ok64 = ok64 && h[t * 16 + k] == (unsigned)(((a + 8 * (t & 1)) << 16) | ((c >> 1) + 2 * k));
-    for (int k = 0; k < 2; ++k) for (int e = 0; e < 2; ++e) ok128 = ok128 && h[t * 16 + 4 + 2 * k + e] == (unsigned)(((a + 8 * e) << 16) | (c + 4 * k));
-    for (int e = 0; e < 2; ++e) for (int i = 0; i < 2; ++i) ok256 = ok256 && h[t * 16 + 8 + 2 * e + i] == (unsigned)(((a + 8 * e) << 16) | (2 * c + i));
-  }
-  printf("  tmem shapes (thread t = 4a + c reads TMEM written by 32x32b with thread = lane, register = column):\n");
-  printf("    16x64b.x2 : register k     <- (lane a + 8*(t&1), column (c>>1) + 2k)      %s\n", ok64 ? "verified" : "MISMATCH");
-  printf("    16x128b.x2: register 2k+e  <- (lane a + 8e,      column c + 4k)           %s\n", ok128 ? "verified" : "MISMATCH");
-  printf("    16x256b.x1: register 2e+i  <- (lane a + 8e,      column 2c + i)           %s\n", ok256 ? "verified" : "MISMATCH");
-  cudaFree(d);
-}
-
 int main(){
   cudaDeviceProp p; CK(cudaGetDeviceProperties(&p,0)); printf("%s SMs=%d L2=%d MB clock=%d MHz\n",p.name,p.multiProcessorCount,p.l2CacheSize>>20,p.clockRate/1000);
   size_t n=(size_t)1<<30; // 1 GiB
@@ -420,9 +270,6 @@ int main(){
     run_alt<double, 4096, 2, 1>(hz); run_alt<double, 4096, 1, 2>(hz);
     run_alt<float, 2048, 8, 1>(hz); run_alt<float, 2048, 4, 2>(hz); run_alt<float, 4096, 4, 1>(hz); run_alt<float, 4096, 2, 2>(hz);
     run_overlap<8, 0, 16>(hz); run_overlap<0, 8, 16>(hz); run_overlap<8, 8, 16>(hz); run_overlap<8, 8, 4>(hz);
-    run_shfl<64, 0, 16>(hz); run_shfl<0, 8, 16>(hz); run_shfl<64, 8, 16>(hz);
-    run_tmem<8, 0>(hz); run_tmem<0, 8>(hz); run_tmem<8, 8>(hz);
-    run_tmemprobe();
   }
   return 0;
 }

@@ -7,16 +7,24 @@
 //  -> [x mid[k]]                                (transfer function H1 / output chirp / 1/N / signs)
 //  -> inverse FFT                               (MODE_CONV only)
 //  -> [x scale] [x rowfac[row]]               (row pass: the y-part of the input chirp, constant along a row)
+//  -> MODE_CONV2 only: the optic of the NEXT surface -- [optic phasor] [x lens2[n] x lens2[line]] -- and a second
+//     convolution FFT -> x mid2[k] -> inverse FFT (fused trains, see fresnel_system_run)
 // and writes the line back in place.  Angular-spectrum propagation is MODE_CONV over rows then
 // over columns (H is separable); fft2d and direct Fresnel are MODE_FWD/MODE_INV over rows then
 // columns.  Shifts are folded into the tables ((-1)^n signs) and never touch memory.
+//
+// MODE_CONV2 (train-level fusion).  The row and the column convolution of a surface commute, so a train
+// of angular-spectrum surfaces can be ordered  rows_0 | cols_0, optic_1, cols_1 | rows_1, optic_2, rows_2 | ...:
+// the last convolution of surface s-1 and the first of surface s run along the same direction and, with the
+// optic of surface s between them, on ONE resident line -- n+1 passes over the wavefront instead of 2n.
 #pragma once
+#include <atomic>
 #include <cstdint>
 #include "fft_core.cuh"
 
 namespace fresnel {
 
-enum PassMode { MODE_FWD = 0, MODE_INV = 1, MODE_CONV = 2 };
+enum PassMode { MODE_FWD = 0, MODE_INV = 1, MODE_CONV = 2, MODE_CONV2 = 3 };
 
 template <typename T> struct PassArgs {
     using C = typename cplx_of<T>::type;
@@ -31,6 +39,11 @@ template <typename T> struct PassArgs {
     T scale;                  // applied last when != 1
     int prefetch_distance;    // tiles ahead to prefetch into L2 (0: off); ~ number of resident CTAs
     int pdl;                  // launched with programmatic stream serialization
+    // MODE_CONV2: the optic between the two convolutions and the second transfer function
+    const C *lens2;           // [batch][N] lens chirp of the in-between optic (applied as lens2[n] * lens2[line]) or nullptr
+    const C *mid2;            // [batch][N] transfer function (with 1/N) of the second convolution
+    const T *amp2;            // [N][N] or nullptr.  TMA column pass: only null / non-null matters (the tile comes
+    const T *opd2;            //                     through the tensor maps given to the launcher)
 };
 
 // Programmatic dependent launch: every pass kernel depends on ALL of the previous pass (a 2-D transform is
@@ -54,6 +67,21 @@ cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t sme
     cfg.attrs = at;
     cfg.numAttrs = pdl ? 1 : 0;
     return cudaLaunchKernelEx(&cfg, kern, args...);
+}
+
+// cudaFuncSetAttribute(MaxDynamicSharedMemorySize) is a per-device setting: every launcher keeps one bit per
+// device ordinal (setting the attribute twice is harmless, so two threads racing here are too)
+inline bool fr_needs_configuring(const std::atomic<unsigned long long> &mask)
+{
+    int dev = 0;
+    cudaGetDevice(&dev);
+    return !((mask.load(std::memory_order_acquire) >> (dev & 63)) & 1ull);
+}
+inline void fr_mark_configured(std::atomic<unsigned long long> &mask)
+{
+    int dev = 0;
+    cudaGetDevice(&dev);
+    mask.fetch_or(1ull << (dev & 63), std::memory_order_release);
 }
 
 // bulk L2 prefetch of a contiguous range (bytes: multiple of 16)
@@ -113,7 +141,7 @@ template <typename T> FR_DEV typename cplx_of<T>::type phasor_turns(T u)
 // v[r] *= exp(2 pi i * opd[r*stride] * inv_lambda), r = 0..15: polynomial for all sixteen, then the rare
 // large phases one by one
 template <typename T>
-FR_DEV void apply_opd16(typename cplx_of<T>::type (&v)[16], const T *__restrict__ o, int stride, T inv_lambda)
+FR_DEV void apply_opd16(typename cplx_of<T>::type (&v)[16], const T *__restrict__ o, size_t stride, T inv_lambda)
 {
     T u[16];
     bool all_small = true;
@@ -167,6 +195,13 @@ __global__ void __launch_bounds__(W *(N / 16), MINB) pass_kernel(PassArgs<T> a)
             }
         }
     }
+    if constexpr (!COL && MODE == MODE_CONV2) {
+        // the map rows of the in-between optic are needed one convolution from now: ask L2 for them
+        if (j == 0) {
+            if (a.opd2 != nullptr) l2_prefetch_bulk(a.opd2 + (size_t)idx * N, (uint32_t)(N * sizeof(T)));
+            if (a.amp2 != nullptr) l2_prefetch_bulk(a.amp2 + (size_t)idx * N, (uint32_t)(N * sizeof(T)));
+        }
+    }
     if constexpr (!COL) {
         if (a.opd != nullptr) {
             apply_opd16<T>(v, a.opd + (size_t)idx * N + j, TL, (T)a.inv_lambda[b]);
@@ -195,7 +230,7 @@ __global__ void __launch_bounds__(W *(N / 16), MINB) pass_kernel(PassArgs<T> a)
         for (int r = 0; r < 16; ++r) v[r] = cmul(v[r], ldg_c(m + j + r * TL));
     }
 
-    if constexpr (MODE == MODE_CONV) fft_line<T, N, +1, COL, W>(v, buf, line, j, a.tw);
+    if constexpr (MODE == MODE_CONV || MODE == MODE_CONV2) fft_line<T, N, +1, COL, W>(v, buf, line, j, a.tw);
 
     if (a.scale != (T)1) {
 #pragma unroll
@@ -209,6 +244,32 @@ __global__ void __launch_bounds__(W *(N / 16), MINB) pass_kernel(PassArgs<T> a)
 #pragma unroll
             for (int r = 0; r < 16; ++r) v[r] = cmul(v[r], c);
         }
+    }
+    if constexpr (MODE == MODE_CONV2) {
+        // the optic of the next surface on the resident line, then its convolution along this same direction
+        const size_t mstride = COL ? (size_t)TL * N : (size_t)TL;
+        const size_t m0 = COL ? (size_t)j * N + idx : (size_t)idx * N + j;
+        if (a.opd2 != nullptr) apply_opd16<T>(v, a.opd2 + m0, mstride, (T)a.inv_lambda[b]);
+        if (a.amp2 != nullptr) {
+#pragma unroll
+            for (int r = 0; r < 16; ++r) {
+                T s = a.amp2[m0 + r * mstride];
+                v[r].x *= s; v[r].y *= s;
+            }
+        }
+        if (a.lens2 != nullptr) {
+            const C *l = a.lens2 + (size_t)b * N;
+            const C c = ldg_c(l + idx);
+#pragma unroll
+            for (int r = 0; r < 16; ++r) v[r] = cmul(v[r], cmul(ldg_c(l + j + r * TL), c));
+        }
+        fft_line<T, N, -1, COL, W>(v, buf, line, j, a.tw);
+        {
+            const C *m = a.mid2 + (size_t)b * N;
+#pragma unroll
+            for (int r = 0; r < 16; ++r) v[r] = cmul(v[r], ldg_c(m + j + r * TL));
+        }
+        fft_line<T, N, +1, COL, W>(v, buf, line, j, a.tw);
     }
 #pragma unroll
     for (int r = 0; r < 16; ++r) g[(size_t)(j + r * TL) * gstride] = v[r];
@@ -273,11 +334,11 @@ cudaError_t launch_pass(const PassArgs<T> &a, int batch, cudaStream_t stream)
 {
     using G = PassGeom<T, N, COL>;
     auto kern = pass_kernel<T, N, COL, G::W, MODE, G::MINB>;
-    static bool configured = false;     // per instantiation; attribute is per-device but we target one GPU per process
-    if (!configured) {
+    static std::atomic<unsigned long long> configured{0};      // one bit per device: the attribute is per device
+    if (fr_needs_configuring(configured)) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::smem);
         if (e != cudaSuccess) return e;
-        configured = true;
+        fr_mark_configured(configured);
     }
     dim3 grid(N / G::W, batch, 1);
     PassArgs<T> b = a;

@@ -19,8 +19,8 @@
 
 namespace fresnel {
 
-constexpr int kBuildMaxBatch = 16;   // batch elements per builder launch (kernel-parameter budget)
-constexpr int kBuildMaxTables = 2;   // tables per builder launch
+constexpr int kBuildMaxBatch = 16;   // batch elements per builder launch (kernel-parameter budget: 4 KB)
+constexpr int kBuildMaxTables = 6;   // tables per builder launch (a fused train builds all its tables up front)
 
 struct ChirpSpec {
     double c_hi, c_lo;   // turns per index^2 (double-double)

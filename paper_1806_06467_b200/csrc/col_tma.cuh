@@ -81,6 +81,10 @@ constexpr int kTmaBoxRows = 256;
 template <typename T, int W> struct MapTile {
     static constexpr int ROW_BYTES = (W * (int)sizeof(T) < 16) ? 16 : W * (int)sizeof(T);
     static constexpr int BOX_COLS = ROW_BYTES / (int)sizeof(T);
+    // A box has to START on a 16-byte boundary of the map row (measured: an 8-byte-aligned start is an illegal
+    // instruction), so a tile narrower than the box takes the aligned box around it and reads at an offset.
+    static __device__ __forceinline__ int box_x(int col0) { return col0 & ~(BOX_COLS - 1); }
+    static __device__ __forceinline__ int col_in_box(int col0, int g) { return (col0 & (BOX_COLS - 1)) + g; }
 };
 
 template <typename T, int N, int W>
@@ -92,11 +96,26 @@ FR_DEV void fetch_map_tile(unsigned char *tile, const CUtensorMap *mmap, uint64_
     if (tid == 0) {
         mbar_expect_tx(bar, (uint32_t)(N * MT::ROW_BYTES));
 #pragma unroll 1
-        for (int r0 = 0; r0 < N; r0 += kTmaBoxRows) tma_load_2d(tile + (size_t)r0 * MT::ROW_BYTES, mmap, bar, col0, r0);
+        for (int r0 = 0; r0 < N; r0 += kTmaBoxRows) tma_load_2d(tile + (size_t)r0 * MT::ROW_BYTES, mmap, bar, MT::box_x(col0), r0);
     }
     mbar_wait(bar, parity);
     parity ^= 1u;
 }
+
+// Fused column pass: where MINB resident CTAs still fit with it, the FIRST map of the in-between optic gets a
+// landing zone of its own behind the tile and is fetched at kernel start (it is an input, not a result of the
+// previous pass, so the fetch does not even wait for it): no bubble between the two convolutions.  Elsewhere
+// (N >= 4096) the map is fetched into the idle exchange space when it is needed.
+template <typename T, int N, int W, int MINB> struct ColMapBuf {
+    static constexpr int ES = (int)sizeof(typename cplx_of<T>::type);
+    static constexpr size_t tile_bytes = ((size_t)W * fr_padded_len(N) * ES + 127) / 128 * 128;
+    static constexpr size_t map_bytes = (size_t)N * MapTile<T, W>::ROW_BYTES;
+#ifdef FR_NO_MAPBUF      // tuning / debugging builds only
+    static constexpr bool enabled = false;
+#else
+    static constexpr bool enabled = (size_t)MINB * (tile_bytes + map_bytes + 1024 + 64) <= (size_t)227 * 1024;
+#endif
+};
 
 template <typename T, int N, int W, int MODE, int MINB>
 __global__ void __launch_bounds__(W *(N / 16), MINB)
@@ -110,6 +129,8 @@ col_tma_kernel(PassArgs<T> a, const __grid_constant__ CUtensorMap tmap, const __
     constexpr int GT = (W == 1) ? 0 : TL;            // group barrier size (W == 1: the CTA is the group)
     extern __shared__ __align__(1024) unsigned char fr_smem[];
     __shared__ __align__(8) uint64_t full_bar;
+    __shared__ __align__(8) uint64_t map_bar;
+    constexpr bool MAPBUF = MODE == MODE_CONV2 && ColMapBuf<T, N, W, MINB>::enabled;
     // 1024-byte alignment (the TMA swizzle pattern is a function of the shared-memory address)
     unsigned char *tile = fr_smem + ((1024u - (smem_u32(fr_smem) & 1023u)) & 1023u);   // landing zone, later the exchange buffers
     C *buf = reinterpret_cast<C *>(tile);
@@ -120,9 +141,22 @@ col_tma_kernel(PassArgs<T> a, const __grid_constant__ CUtensorMap tmap, const __
     const int b = blockIdx.y;
     const int col0 = blockIdx.x * W;
 
-    if (tid == 0) mbar_init(&full_bar, 1);
+    if (tid == 0) {
+        mbar_init(&full_bar, 1);
+        if constexpr (MAPBUF) mbar_init(&map_bar, 1);
+    }
     pdl_launch_dependents();
     __syncthreads();
+    if constexpr (MAPBUF) {
+        if (tid == 0 && (a.opd2 != nullptr || a.amp2 != nullptr)) {
+            using MT = MapTile<T, W>;
+            unsigned char *mapbuf = tile + ColMapBuf<T, N, W, MINB>::tile_bytes;
+            const CUtensorMap *mm = a.opd2 != nullptr ? &tmap_opd2 : &tmap_amp2;
+            mbar_expect_tx(&map_bar, (uint32_t)(N * MT::ROW_BYTES));
+#pragma unroll 1
+            for (int r0 = 0; r0 < N; r0 += kTmaBoxRows) tma_load_2d(mapbuf + (size_t)r0 * MT::ROW_BYTES, mm, &map_bar, MT::box_x(col0), r0);
+        }
+    }
     pdl_wait();                                      // the row pass has finished: the wavefront may be read
     if (tid == 0) {
         mbar_expect_tx(&full_bar, (uint32_t)(N * ROW_BYTES));
@@ -156,63 +190,52 @@ col_tma_kernel(PassArgs<T> a, const __grid_constant__ CUtensorMap tmap, const __
 #pragma unroll
         for (int r = 0; r < 16; ++r) v[r] = cmul(v[r], ldg_c(p + j + r * TL));
     }
-    if constexpr (MODE == MODE_INV) fft_line<T, N, +1, false, W, GT>(v, buf, g, j, a.tw, 1 + g);
-    else                            fft_line<T, N, -1, false, W, GT>(v, buf, g, j, a.tw, 1 + g);
-    if (a.mid != nullptr) {
-        const C *m = a.mid + (size_t)b * N;
-#pragma unroll
-        for (int r = 0; r < 16; ++r) v[r] = cmul(v[r], ldg_c(m + j + r * TL));
-    }
-    if constexpr (MODE == MODE_CONV || MODE == MODE_CONV2) fft_line<T, N, +1, false, W, GT>(v, buf, g, j, a.tw, 1 + g);
-    if (a.scale != (T)1) {
-#pragma unroll
-        for (int r = 0; r < 16; ++r) { v[r].x *= a.scale; v[r].y *= a.scale; }
-    }
-    if constexpr (MODE == MODE_CONV2) {
-        // the optic of the next surface on the resident tile (its maps arrive by TMA in the exchange space, which is
-        // idle between the two convolutions), then that surface's column convolution
+    line_transforms<T, N, MODE, false, W, GT>(v, buf, g, j, b, a, 1 + g, [&](C (&u)[16]) {
+        // MODE_CONV2: the optic of the next surface on the resident tile; its maps arrive by TMA in the exchange
+        // space, which is idle between the two convolutions
         using MT = MapTile<T, W>;
         uint32_t parity = 1;                         // phase 0 was the wavefront tile
+        const unsigned char *mt = tile;              // where the current map tile is read from
+        bool synced = false;                         // a CTA-wide sync is owed before the exchange space is reused
         if (a.opd2 != nullptr) {
-            fetch_map_tile<T, N, W>(tile, &tmap_opd2, &full_bar, parity, col0, tid);
+            if constexpr (MAPBUF) { mbar_wait(&map_bar, 0); mt = tile + ColMapBuf<T, N, W, MINB>::tile_bytes; }
+            else { fetch_map_tile<T, N, W>(tile, &tmap_opd2, &full_bar, parity, col0, tid); synced = true; }
             const T il = (T)a.inv_lambda[b];
-            T u[16];
+            T ph[16];
             bool all_small = true;
 #pragma unroll
             for (int r = 0; r < 16; ++r) {
-                u[r] = *reinterpret_cast<const T *>(tile + (size_t)(j + r * TL) * MT::ROW_BYTES + g * sizeof(T)) * il;
-                all_small = all_small && phasor_is_small(u[r]);
+                ph[r] = *reinterpret_cast<const T *>(mt + (size_t)(j + r * TL) * MT::ROW_BYTES + MT::col_in_box(col0, g) * sizeof(T)) * il;
+                all_small = all_small && phasor_is_small(ph[r]);
             }
             if (all_small) {
 #pragma unroll
-                for (int r = 0; r < 16; ++r) v[r] = cmul(v[r], phasor_turns_small(u[r]));
+                for (int r = 0; r < 16; ++r) u[r] = cmul(u[r], phasor_turns_small(ph[r]));
             } else {
 #pragma unroll
-                for (int r = 0; r < 16; ++r) v[r] = cmul(v[r], phasor_turns_any(u[r]));
+                for (int r = 0; r < 16; ++r) u[r] = cmul(u[r], phasor_turns_any(ph[r]));
             }
         }
         if (a.amp2 != nullptr) {
-            fetch_map_tile<T, N, W>(tile, &tmap_amp2, &full_bar, parity, col0, tid);
+            if (MAPBUF && a.opd2 == nullptr) { mbar_wait(&map_bar, 0); mt = tile + ColMapBuf<T, N, W, MINB>::tile_bytes; }
+            else { fetch_map_tile<T, N, W>(tile, &tmap_amp2, &full_bar, parity, col0, tid); mt = tile; synced = true; }
 #pragma unroll
             for (int r = 0; r < 16; ++r) {
-                const T s = *reinterpret_cast<const T *>(tile + (size_t)(j + r * TL) * MT::ROW_BYTES + g * sizeof(T));
-                v[r].x *= s; v[r].y *= s;
+                const T s = *reinterpret_cast<const T *>(mt + (size_t)(j + r * TL) * MT::ROW_BYTES + MT::col_in_box(col0, g) * sizeof(T));
+                u[r].x *= s; u[r].y *= s;
             }
         }
-        if (a.opd2 != nullptr || a.amp2 != nullptr) __syncthreads();      // the map tile has been read: exchange space again
+        if (synced) __syncthreads();                 // a map tile was read from the exchange space: release it
         if (a.lens2 != nullptr) {
             const C *l = a.lens2 + (size_t)b * N;
             const C c = ldg_c(l + col0 + g);
 #pragma unroll
-            for (int r = 0; r < 16; ++r) v[r] = cmul(v[r], cmul(ldg_c(l + j + r * TL), c));
+            for (int r = 0; r < 16; ++r) u[r] = cmul(u[r], cmul(ldg_c(l + j + r * TL), c));
         }
-        fft_line<T, N, -1, false, W, GT>(v, buf, g, j, a.tw, 1 + g);
-        {
-            const C *m = a.mid2 + (size_t)b * N;
+    });
+    if (a.scale != (T)1) {
 #pragma unroll
-            for (int r = 0; r < 16; ++r) v[r] = cmul(v[r], ldg_c(m + j + r * TL));
-        }
-        fft_line<T, N, +1, false, W, GT>(v, buf, g, j, a.tw, 1 + g);
+        for (int r = 0; r < 16; ++r) { v[r].x *= a.scale; v[r].y *= a.scale; }
     }
 
     __syncthreads();                                 // every group is done with its exchange buffer
@@ -259,6 +282,9 @@ template <typename T, int N> struct ColTmaGeom {
     static constexpr int minb0 = minb_regs < minb_smem ? minb_regs : minb_smem;
     static constexpr int MINB = minb0 < 1 ? 1 : (minb0 > 8 ? 8 : minb0);
     static constexpr bool supported = TL >= 32;      // named barriers work on whole warps
+    // dynamic shared memory of the fused (MODE_CONV2) kernel: tile + alignment slack [+ map landing zone]
+    static constexpr size_t smem_conv2 = ColMapBuf<T, N, W, MINB>::enabled
+        ? ColMapBuf<T, N, W, MINB>::tile_bytes + ColMapBuf<T, N, W, MINB>::map_bytes + 1024 : smem + 1024;
 };
 
 // tmap: the wavefront; tmap_amp2 / tmap_opd2: the maps of the in-between optic (MODE_CONV2; read only when
@@ -272,16 +298,17 @@ cudaError_t launch_col_tma(const PassArgs<T> &a, const CUtensorMap &tmap, const 
         return cudaErrorNotSupported;
     } else {
         auto kern = col_tma_kernel<T, N, G::W, MODE, G::MINB>;
+        constexpr size_t dyn_smem = MODE == MODE_CONV2 ? G::smem_conv2 : G::smem + 1024;
         static std::atomic<unsigned long long> configured{0};
         if (fr_needs_configuring(configured)) {
-            cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::smem + 1024);
+            cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn_smem);
             if (e != cudaSuccess) return e;
             fr_mark_configured(configured);
         }
         dim3 grid(N / G::W, batch, 1);
         PassArgs<T> b = a;
         if (b.prefetch_distance < 0) b.prefetch_distance = -b.prefetch_distance * G::MINB;
-        return launch_pdl(kern, grid, dim3(G::threads), G::smem + 1024, stream, b.pdl != 0, b, tmap, tmap_amp2, tmap_opd2);
+        return launch_pdl(kern, grid, dim3(G::threads), dyn_smem, stream, b.pdl != 0, b, tmap, tmap_amp2, tmap_opd2);
     }
 }
 

@@ -159,6 +159,64 @@ FR_DEV void apply_opd16(typename cplx_of<T>::type (&v)[16], const T *__restrict_
     }
 }
 
+// The transforms of one resident line, for every mode, as a ROLLED loop over ONE copy of the forward transform:
+// an inverse transform is conj o forward o conj, and the conjugations fold into the neighbouring multiplies
+// (bit-identical to a transform with conjugated twiddles: negation is exact).  One copy keeps the instruction
+// footprint at a quarter of the unrolled fused kernel, and -- what matters -- keeps ptxas from spilling: four
+// inlined transforms cost 150-350 bytes of spill traffic per thread on the load/store pipe the exchanges need.
+//   MODE_FWD   F, [x mid]                         MODE_INV   conj, F, conj, [x mid]
+//   MODE_CONV  F, x mid, conj, F, conj            MODE_CONV2 the same twice, optic2(v) in between, then mid2
+template <typename T, int N, int MODE, bool COL, int W, int GT, typename Optic2>
+FR_DEV void line_transforms(typename cplx_of<T>::type (&v)[16], typename cplx_of<T>::type *buf, int line, int j, int b,
+                            const PassArgs<T> &a, int bar_id, Optic2 &&optic2)
+{
+    using C = typename cplx_of<T>::type;
+    constexpr int TL = N / 16;
+    constexpr int NIT = MODE == MODE_CONV2 ? 4 : (MODE == MODE_CONV ? 2 : 1);
+    const C *m = a.mid != nullptr ? a.mid + (size_t)b * N : nullptr;
+    if constexpr (MODE == MODE_INV) {
+#pragma unroll
+        for (int r = 0; r < 16; ++r) v[r].y = -v[r].y;
+    }
+#pragma unroll 1
+    for (int it = 0; it < NIT; ++it) {
+        fft_line<T, N, -1, COL, W, GT>(v, buf, line, j, a.tw, bar_id);
+        if constexpr (MODE == MODE_FWD) {
+            if (m != nullptr) {
+#pragma unroll
+                for (int r = 0; r < 16; ++r) v[r] = cmul(v[r], ldg_c(m + j + r * TL));
+            }
+        } else if constexpr (MODE == MODE_INV) {
+            if (m != nullptr) {
+#pragma unroll
+                for (int r = 0; r < 16; ++r) v[r] = cmulc(ldg_c(m + j + r * TL), v[r]);      // mid * conj(v)
+            } else {
+#pragma unroll
+                for (int r = 0; r < 16; ++r) v[r].y = -v[r].y;
+            }
+        } else if ((it & 1) == 0) {
+            // x transfer function, conjugated for the inverse transform that follows.  (m is never null here; the
+            // branch keeps the 16 table loads from being hoisted into the transform, where they would cost registers)
+            if (m != nullptr) {
+#pragma unroll
+                for (int r = 0; r < 16; ++r) {
+                    const C t = cmul(v[r], ldg_c(m + j + r * TL));
+                    v[r].x = t.x; v[r].y = -t.y;
+                }
+            }
+        } else {
+#pragma unroll
+            for (int r = 0; r < 16; ++r) v[r].y = -v[r].y;
+            if constexpr (MODE == MODE_CONV2) {
+                if (it == 1) {
+                    optic2(v);
+                    m = a.mid2 + (size_t)b * N;
+                }
+            }
+        }
+    }
+}
+
 template <typename T, int N, bool COL, int W, int MODE, int MINB>
 __global__ void __launch_bounds__(W *(N / 16), MINB) pass_kernel(PassArgs<T> a)
 {
@@ -221,16 +279,25 @@ __global__ void __launch_bounds__(W *(N / 16), MINB) pass_kernel(PassArgs<T> a)
         for (int r = 0; r < 16; ++r) v[r] = cmul(v[r], ldg_c(p + j + r * TL));
     }
 
-    if constexpr (MODE == MODE_INV) fft_line<T, N, +1, COL, W>(v, buf, line, j, a.tw);
-    else                            fft_line<T, N, -1, COL, W>(v, buf, line, j, a.tw);
-
-    if (a.mid != nullptr) {
-        const C *m = a.mid + (size_t)b * N;
+    line_transforms<T, N, MODE, COL, W, 0>(v, buf, line, j, b, a, 0, [&](C (&u)[16]) {
+        // MODE_CONV2: the optic of the next surface on the resident line
+        const size_t mstride = COL ? (size_t)TL * N : (size_t)TL;
+        const size_t m0 = COL ? (size_t)j * N + idx : (size_t)idx * N + j;
+        if (a.opd2 != nullptr) apply_opd16<T>(u, a.opd2 + m0, mstride, (T)a.inv_lambda[b]);
+        if (a.amp2 != nullptr) {
 #pragma unroll
-        for (int r = 0; r < 16; ++r) v[r] = cmul(v[r], ldg_c(m + j + r * TL));
-    }
-
-    if constexpr (MODE == MODE_CONV || MODE == MODE_CONV2) fft_line<T, N, +1, COL, W>(v, buf, line, j, a.tw);
+            for (int r = 0; r < 16; ++r) {
+                T s = a.amp2[m0 + r * mstride];
+                u[r].x *= s; u[r].y *= s;
+            }
+        }
+        if (a.lens2 != nullptr) {
+            const C *l = a.lens2 + (size_t)b * N;
+            const C c = ldg_c(l + idx);
+#pragma unroll
+            for (int r = 0; r < 16; ++r) u[r] = cmul(u[r], cmul(ldg_c(l + j + r * TL), c));
+        }
+    });
 
     if (a.scale != (T)1) {
 #pragma unroll
@@ -244,32 +311,6 @@ __global__ void __launch_bounds__(W *(N / 16), MINB) pass_kernel(PassArgs<T> a)
 #pragma unroll
             for (int r = 0; r < 16; ++r) v[r] = cmul(v[r], c);
         }
-    }
-    if constexpr (MODE == MODE_CONV2) {
-        // the optic of the next surface on the resident line, then its convolution along this same direction
-        const size_t mstride = COL ? (size_t)TL * N : (size_t)TL;
-        const size_t m0 = COL ? (size_t)j * N + idx : (size_t)idx * N + j;
-        if (a.opd2 != nullptr) apply_opd16<T>(v, a.opd2 + m0, mstride, (T)a.inv_lambda[b]);
-        if (a.amp2 != nullptr) {
-#pragma unroll
-            for (int r = 0; r < 16; ++r) {
-                T s = a.amp2[m0 + r * mstride];
-                v[r].x *= s; v[r].y *= s;
-            }
-        }
-        if (a.lens2 != nullptr) {
-            const C *l = a.lens2 + (size_t)b * N;
-            const C c = ldg_c(l + idx);
-#pragma unroll
-            for (int r = 0; r < 16; ++r) v[r] = cmul(v[r], cmul(ldg_c(l + j + r * TL), c));
-        }
-        fft_line<T, N, -1, COL, W>(v, buf, line, j, a.tw);
-        {
-            const C *m = a.mid2 + (size_t)b * N;
-#pragma unroll
-            for (int r = 0; r < 16; ++r) v[r] = cmul(v[r], ldg_c(m + j + r * TL));
-        }
-        fft_line<T, N, +1, COL, W>(v, buf, line, j, a.tw);
     }
 #pragma unroll
     for (int r = 0; r < 16; ++r) g[(size_t)(j + r * TL) * gstride] = v[r];

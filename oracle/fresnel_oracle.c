@@ -24,7 +24,11 @@
  *   - "direct Fresnel" single-FFT propagation, pixelscale changes:
  *   - fftshift puts the origin in the centre of the array:
  *
- * Parity pins: every function here is pinned in tests/test_oracle_pins.py (P0..P13 of
+ * Grid sizes: any N >= 2.  Powers of two go through the radix-2 FFT; every other N (the paper
+ * ran N = 2800; App. B gives npix = 1025, :259) through the plain separable
+ * O(N^3) DFT of item 2b -- no FFT cleverness for those.
+ *
+ * Parity pins: every function here is pinned in tests/test_oracle_pins.py (P0..P19 of
  * DESIGN.md) against closed forms / exact identities / brute force.  Nothing is
  * "parity unpinned".
  */
@@ -143,11 +147,85 @@ static void fft1d_radix2(double *x, int n, const double *tw)
     }
 }
 
+/* ------------------------------------------------------------------------------------------
+ * 2b. dft2_any: the separable DFT for ANY N, written out as its definition -- rows, then columns,
+ *     each 1-D transform the plain O(N^2) sum
+ *         out[p] = sum_k in[k] * w[(k*p) mod N],   w[m] = exp(sign*2*pi*i*m/N) from direct cosl/sinl,
+ *     accumulated in double.  O(N^3) in total; used for every N that is not a power of two
+ *     (SURVEY.md sec. 8(f) NEXT-2; PAPER.md:137, :172 N = 2800; :259 npix = 1025).
+ * ------------------------------------------------------------------------------------------ */
+static void dft1d_plain(const double *in, double *out, int n, int stride, const double *w)
+{
+    for (int p = 0; p < n; ++p) {
+        double sr = 0.0, si = 0.0;
+        long m = 0;                                /* (k*p) mod n, advanced by p per term */
+        for (int k = 0; k < n; ++k) {
+            const double ar = in[2 * (size_t)k * stride], ai = in[2 * (size_t)k * stride + 1];
+            sr += ar * w[2 * m] - ai * w[2 * m + 1];
+            si += ar * w[2 * m + 1] + ai * w[2 * m];
+            m += p;
+            if (m >= n) m -= n;
+        }
+        out[2 * p] = sr;
+        out[2 * p + 1] = si;
+    }
+}
+
+static int dft2_any_core(double *u, int N, int sign, int normalise)
+{
+    if (!u || N < 1 || (sign != 1 && sign != -1)) return ORACLE_ERR_INVALID_ARG;
+    double *w = (double *)malloc(2 * (size_t)N * sizeof(double));
+    if (!w) return ORACLE_ERR_ALLOC;
+    for (int m = 0; m < N; ++m) {
+        long double a = (long double)sign * 2.0L * PI_L * (long double)m / (long double)N;
+        w[2 * m] = (double)cosl(a);
+        w[2 * m + 1] = (double)sinl(a);
+    }
+    int fail = 0;
+#pragma omp parallel num_threads(nthreads())
+    {
+        double *line = (double *)malloc(2 * (size_t)N * sizeof(double));
+        if (!line) {
+#pragma omp atomic write
+            fail = 1;
+        }
+#pragma omp barrier
+        if (!fail) {
+#pragma omp for schedule(static)
+            for (int j = 0; j < N; ++j) {                       /* rows */
+                dft1d_plain(u + 2 * (size_t)j * N, line, N, 1, w);
+                memcpy(u + 2 * (size_t)j * N, line, 2 * (size_t)N * sizeof(double));
+            }
+#pragma omp for schedule(static)
+            for (int k = 0; k < N; ++k) {                       /* columns */
+                dft1d_plain(u + 2 * (size_t)k, line, N, N, w);
+                for (int j = 0; j < N; ++j) {
+                    u[2 * ((size_t)j * N + k)] = line[2 * j];
+                    u[2 * ((size_t)j * N + k) + 1] = line[2 * j + 1];
+                }
+            }
+            if (normalise) {
+                double sc = 1.0 / ((double)N * (double)N);
+#pragma omp for schedule(static)
+                for (int j = 0; j < N; ++j)
+                    for (int k = 0; k < 2 * N; ++k) u[2 * (size_t)j * N + k] *= sc;
+            }
+        }
+        free(line);
+    }
+    free(w);
+    return fail ? ORACLE_ERR_ALLOC : ORACLE_OK;
+}
+
+/* forward (sign=-1) unnormalised; inverse (sign=+1) scaled by 1/N^2; any N >= 1. */
+int oracle_dft2_any(double *u, int N, int sign) { return dft2_any_core(u, N, sign, sign > 0); }
+
 /* normalise != 0: multiply by 1/N^2 (only meaningful with sign = +1). */
 static int fft2_core(double *u, int N, int sign, int normalise)
 {
     if (!u || (sign != 1 && sign != -1)) return ORACLE_ERR_INVALID_ARG;
-    if (!is_pow2(N) || N < 2) return ORACLE_ERR_UNSUPPORTED;
+    if (N < 2) return ORACLE_ERR_UNSUPPORTED;
+    if (!is_pow2(N)) return dft2_any_core(u, N, sign, normalise);
     double *tw = (double *)malloc((size_t)N * sizeof(double));
     if (!tw) return ORACLE_ERR_ALLOC;
     make_twiddles(tw, N, sign);
@@ -282,23 +360,22 @@ int oracle_apply_mask(double *u, int N, const double *amp, const double *opd, do
 
 /* ------------------------------------------------------------------------------------------
  * 5. propagate_as: the literal sequence  ifftshift -> fft2(-) -> x H -> fft2(+) -> fftshift
- *      H[p,q] = exp(-i*pi*lambda*z*(f_q^2 + f_p^2)),  f in FFT order: f_q = q/(N dx) (q < N/2),
- *      (q-N)/(N dx) otherwise.  No piston exp(ikz) (g5).  z = 0 is the identity (g11).
+ *      H[p,q] = exp(-i*pi*lambda*z*(f_q^2 + f_p^2)),  f in FFT order: f_q = q/(N dx) for q < (N+1)/2
+ *      (= N/2 for even N), (q-N)/(N dx) otherwise.  No piston exp(ikz) (g5).  z = 0 is the identity (g11).
  *    ("plane-to-plane angular spectrum propagation"; BASELINE.json:north_star)
  * ------------------------------------------------------------------------------------------ */
 int oracle_propagate_as(double *u, int N, double dx, double lambda, double z)
 {
     if (!u || N <= 0 || !(dx > 0) || !(lambda > 0) || !isfinite(z)) return ORACLE_ERR_INVALID_ARG;
-    if (!is_pow2(N)) return ORACLE_ERR_UNSUPPORTED;
     int rc;
     if ((rc = oracle_ifftshift(u, N)) != ORACLE_OK) return rc;
     if ((rc = oracle_fft2(u, N, -1)) != ORACLE_OK) return rc;
     long double ldx = dx, ll = lambda, lz = z;
 #pragma omp parallel for num_threads(nthreads()) schedule(static)
     for (int p = 0; p < N; ++p) {
-        long double fp = (long double)(p < N / 2 ? p : p - N) / ((long double)N * ldx);
+        long double fp = (long double)(p < (N + 1) / 2 ? p : p - N) / ((long double)N * ldx);
         for (int q = 0; q < N; ++q) {
-            long double fq = (long double)(q < N / 2 ? q : q - N) / ((long double)N * ldx);
+            long double fq = (long double)(q < (N + 1) / 2 ? q : q - N) / ((long double)N * ldx);
             long double th = -PI_L * ll * lz * (fq * fq + fp * fp);
             double c = (double)cosl(th), s = (double)sinl(th);
             double *e = u + 2 * ((size_t)p * N + q);
@@ -321,7 +398,6 @@ int oracle_propagate_direct(double *u, int N, double *dx_inout, double lambda, d
 {
     if (!u || !dx_inout || N <= 0 || !(*dx_inout > 0) || !(lambda > 0) || !isfinite(z) || z == 0.0)
         return ORACLE_ERR_INVALID_ARG;
-    if (!is_pow2(N)) return ORACLE_ERR_UNSUPPORTED;
     double dx = *dx_inout;
     int rc;
     if ((rc = oracle_apply_qpf(u, N, dx, lambda, z)) != ORACLE_OK) return rc;

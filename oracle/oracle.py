@@ -33,6 +33,8 @@ def lib():
         L.oracle_get_threads.restype = ctypes.c_int
         L.oracle_dft2_naive.argtypes = [dp, ctypes.c_int, ctypes.c_int]
         L.oracle_fft2.argtypes = [dp, ctypes.c_int, ctypes.c_int]
+        L.oracle_dft2_any.argtypes = [dp, ctypes.c_int, ctypes.c_int]
+        L.oracle_dft2_any.restype = ctypes.c_int
         L.oracle_fftshift.argtypes = [dp, ctypes.c_int]
         L.oracle_ifftshift.argtypes = [dp, ctypes.c_int]
         L.oracle_fft2d.argtypes = [dp, ctypes.c_int, ctypes.c_int, ctypes.c_int]
@@ -98,6 +100,13 @@ def dft2_naive(u, sign):
 def fft2(u, sign):
     a, N = _prep(u)
     _check(lib().oracle_fft2(_dptr(a), N, int(sign)), "fft2")
+    return a
+
+
+def dft2_any(u, sign):
+    """The plain separable O(N^3) DFT, any N (what fft2 uses when N is not a power of two)."""
+    a, N = _prep(u)
+    _check(lib().oracle_dft2_any(_dptr(a), N, int(sign)), "dft2_any")
     return a
 
 

@@ -460,3 +460,95 @@ def test_p15_system_run_threshold_masks_and_zero_distance(oracle):
     assert oracle.system_run(u0, dx, lam, [Surface(math.inf, zc * (1 - 1e-12))])[2] == [0]
     with pytest.raises(oracle.OracleError):
         oracle.system_run(u0, dx, lam, [Surface(0.0, 0.1)])
+
+
+# ---- P16-P19: grids that are not a power of two (SURVEY.md sec. 8(f) NEXT-2; PAPER.md:137, :172 N = 2800; :259) ----
+@pytest.mark.parametrize("N", [9, 12, 15, 35])
+@pytest.mark.parametrize("sign", [-1, +1])
+def test_P16_dft2_any_vs_bruteforce_and_closed_forms(oracle, N, sign):
+    """The plain separable O(N^3) DFT against the literal O(N^4) double sum at odd, even and composite N, and
+    against closed forms (single exponential -> N^2 at [p0, q0]; shifted delta -> conjugate phase ramp): pins the
+    sign, the axis order, the (k p) mod N indexing and the 1/N^2 of the path every non-power-of-two grid takes."""
+    u = rnd(N, 160 + N)
+    assert rel(oracle.dft2_any(u, sign), oracle.dft2_naive(u, sign)) <= 1e-13
+    assert rel(oracle.fft2(u, sign), oracle.dft2_naive(u, sign)) <= 1e-13          # the dispatch of fft2
+    j, k = np.meshgrid(np.arange(N), np.arange(N), indexing="ij")
+    p0, q0 = 2, N - 3
+    e = np.exp(2j * np.pi * (j * p0 + k * q0) / N)
+    F = oracle.dft2_any(e, -1)
+    expect = np.zeros((N, N), complex)
+    expect[p0, q0] = N * N
+    assert np.abs(F - expect).max() < 1e-10
+    d = np.zeros((N, N), complex)
+    d[1, N - 2] = 1.0
+    assert np.abs(oracle.dft2_any(d, -1) - np.exp(-2j * np.pi * (j * 1 + k * (N - 2)) / N)).max() < 1e-13
+
+
+def test_P16_dft2_any_special_cases(oracle):
+    """At a power of two the plain DFT must agree with the radix-2 path (N = 64); at N = 100 and 175 with the
+    library routine (numpy's mixed-radix FFT); forward then inverse is the identity (1/N^2)."""
+    u = rnd(64, 161)
+    assert rel(oracle.dft2_any(u, -1), oracle.fft2(u, -1)) <= 1e-13
+    for N in (100, 175):
+        u = rnd(N, 162 + N)
+        assert rel(oracle.fft2(u, -1), np.fft.fft2(u)) <= 1e-13
+        assert rel(oracle.fft2(u, +1), np.fft.ifft2(u)) <= 1e-13
+        assert rel(oracle.fft2(oracle.fft2(u, -1), +1), u) <= 1e-13
+
+
+@pytest.mark.parametrize("N", [9, 35, 100])
+def test_P17_shifts_and_centred_transform_any_N(oracle, N):
+    """fftshift / ifftshift are different rotations for odd N (by N//2 and by -(N//2)): exact equality with numpy's,
+    and the centred transform of the ABI equals numpy's fftshift(fft2(ifftshift(u)))."""
+    u = rnd(N, 170 + N)
+    assert np.array_equal(oracle.fftshift(u), np.fft.fftshift(u))
+    assert np.array_equal(oracle.ifftshift(u), np.fft.ifftshift(u))
+    assert np.array_equal(oracle.ifftshift(oracle.fftshift(u)), u)
+    assert rel(oracle.fft2d(u, +1, True), np.fft.fftshift(np.fft.fft2(np.fft.ifftshift(u)))) <= 1e-13
+    assert rel(oracle.fft2d(u, -1, True), np.fft.fftshift(np.fft.ifft2(np.fft.ifftshift(u)))) <= 1e-13
+
+
+@pytest.mark.parametrize("N", [700, 625])
+def test_P18_gaussian_beam_closed_form_any_N(oracle, N):
+    """P4 on a 2^2 5^2 7 grid and on an odd 5^4 grid: the sampled Gaussian beam after angular-spectrum and after
+    direct propagation equals (q0/q) exp(i pi r^2/(lambda q)).  For odd N this pins the frequency order
+    f_q = q/(N dx) for q <= (N-1)/2, (q-N)/(N dx) above (a wrong split moves one frequency from +f to -f-1/(N dx))
+    and the grid centre on pixel N//2."""
+    dx, lam, w0 = 2e-5, 1.064e-6, 1.2e-3
+    u0 = gaussian_closed_form(N, dx, lam, w0, 0.0)
+    for z in (0.4, -0.4):
+        assert rel(oracle.propagate_as(u0, dx, lam, z), gaussian_closed_form(N, dx, lam, w0, z)) <= 1e-9
+    for z in (0.6, -0.6):
+        v, dx1 = oracle.propagate_direct(u0, dx, lam, z)
+        assert dx1 == pytest.approx(lam * abs(z) / (N * dx), rel=1e-15)
+        assert rel(v, gaussian_closed_form(N, dx1, lam, w0, z)) <= 1e-9
+
+
+def test_P19_exact_identities_any_N(oracle):
+    """Exact identities on non-power-of-two grids: Talbot self-imaging (N = 240, period 16 px; also N = 243 = 3^5
+    with period 9 px, an odd grid), the semigroup AS(z1) AS(z2) = AS(z1 + z2), AS(z) AS(-z) = id, Parseval for both
+    propagators, direct(-z) direct(z) = id, and AS == direct at z_c = N dx^2 / lambda (N = 300; for odd N the discrete
+    chirp exp(i pi m^2 / N) is not its own transform -- a Gauss-sum fact -- so that identity is an even-N one)."""
+    dx, lam = 1e-5, 1e-6
+    for N, d in ((240, 16), (243, 9)):
+        j, k = np.meshgrid(np.arange(N), np.arange(N), indexing="ij")
+        u = np.exp(1j * 0.3 * np.cos(2 * np.pi * k / d)) * (1 + 0.2 * np.sin(2 * np.pi * j / d))
+        zT = 2 * (d * dx) ** 2 / lam
+        assert rel(oracle.propagate_as(u, dx, lam, zT), u) <= 1e-12
+    N = 300
+    u = rnd(N, 190)
+    assert rel(oracle.propagate_as(oracle.propagate_as(u, dx, lam, 0.01), dx, lam, 0.02), oracle.propagate_as(u, dx, lam, 0.03)) <= 1e-13
+    assert rel(oracle.propagate_as(oracle.propagate_as(u, dx, lam, 0.02), dx, lam, -0.02), u) <= 1e-13
+    assert np.sum(np.abs(oracle.propagate_as(u, dx, lam, 0.02)) ** 2) == pytest.approx(np.sum(np.abs(u) ** 2), rel=1e-13)
+    v, dx1 = oracle.propagate_direct(u, dx, lam, 0.05)
+    assert np.sum(np.abs(v) ** 2) * dx1 ** 2 == pytest.approx(np.sum(np.abs(u) ** 2) * dx ** 2, rel=1e-13)
+    w, dx2 = oracle.propagate_direct(v, dx1, lam, -0.05)
+    assert dx2 == pytest.approx(dx, rel=1e-15) and rel(w, u) <= 1e-11
+    for N in (300,):
+        x, y = coords(N, 2e-5)
+        g = np.exp(-(x * x + y * y) / (0.8e-3) ** 2) * (1 + 0.05 * np.cos(2 * np.pi * x / 2e-4))
+        zc = N * (2e-5) ** 2 / lam
+        a = oracle.propagate_as(g, 2e-5, lam, zc)
+        b, dxo = oracle.propagate_direct(g, 2e-5, lam, zc)
+        assert dxo == pytest.approx(2e-5, rel=1e-14)
+        assert rel(a, b) <= 1e-9

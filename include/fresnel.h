@@ -30,8 +30,7 @@
  *                FRESNEL_ERR_INVALID_ARG  NULL plan/wf/host array, lambda <= 0, pixel <= 0, non-finite
  *                                         z, z == 0 where a division by z is needed, f == 0 or NaN,
  *                                         bad direction
- *                FRESNEL_ERR_UNSUPPORTED  N not a power of two in [64, 8192] (the paper's N = 2800
- *                                         run, is a later milestone), bad dtype
+ *                FRESNEL_ERR_UNSUPPORTED  grid size outside the supported set (see fresnel_plan_create), bad dtype
  *                FRESNEL_ERR_ALLOC        device/host allocation failed (plan create, fresnel_plan_reserve_tables),
  *                                         or a call needs more chirp-table slots than are free (all taken by
  *                                         captured graphs: see fresnel_plan_reserve_tables)
@@ -66,7 +65,16 @@ enum { FRESNEL_FORWARD = +1, FRESNEL_INVERSE = -1 };
 
 /* Create a plan for `batch` wavefronts of N x N complex elements of `dtype` on the current CUDA
  * device.  Builds the FFT twiddle tables (host long double, rounded once) and allocates the chirp
- * table cache.  N: power of two in [64, 8192]; batch >= 1.  *out is set only on FRESNEL_OK. */
+ * table cache.  batch >= 1.  *out is set only on FRESNEL_OK.  Grid sizes:
+ *   - powers of two in [64, 8192]: the register-resident radix-16 kernels (the fast path; all BASELINE configs);
+ *   - any other N in [16, 8192] ("N = 2800 ran faster than 4096"; npix = 1025, :259): the
+ *     shared-memory path of gen_kernel.cuh -- mixed radix when N = 2^a 3^b 5^c 7^d 11^e 13^f, otherwise Bluestein
+ *     (chirp x circular convolution of the next 7-smooth length >= 2N-1 x chirp), as long as two line buffers of the
+ *     transform length fit one SM's shared memory (complex128: mixed radix N <= 7200, Bluestein N <= 3600;
+ *     complex64: 7200 / 3600 with 16-byte column tiles); beyond that FRESNEL_ERR_UNSUPPORTED.  Odd N: the grid
+ *     centre is pixel N/2 (integer division), frequencies in FFT order are q/(N dx) for q <= (N-1)/2 and
+ *     (q-N)/(N dx) above, and centred transforms carry phase ramps instead of (-1)^n signs.  Train-level fusion
+ *     (fresnel_system_run) applies to power-of-two grids only. */
 fresnel_status fresnel_plan_create(fresnel_plan **out, int N, int batch, fresnel_dtype dtype);
 
 /* Stream all later calls enqueue on (a cudaStream_t passed as void*; NULL = legacy default stream).  The new

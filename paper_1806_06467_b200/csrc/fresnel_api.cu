@@ -13,6 +13,7 @@
 
 #include "../../include/fresnel.h"
 #include "dispatch.h"
+#include "gen_kernel.cuh"
 #include "pointwise.cuh"
 #include "tables.cuh"
 
@@ -79,6 +80,12 @@ struct fresnel_plan {
     int sms = 148;
     int pdl = 1;                        // programmatic dependent launch of the pass kernels (FRESNEL_PDL=0: off, A/B timing)
     int fuse = 1;                       // train-level pass fusion in fresnel_system_run (FRESNEL_FUSE=0: off, A/B timing)
+    // grids that are not a power of two (gen_kernel.cuh): transform length, radices, root table, Bluestein tables
+    bool generic = false;
+    int gen_M = 0, gen_nstages = 0, gen_radix[kGenMaxStages] = {0};
+    int gen_wcol = 1, gen_box_rows = 256;
+    bool gen_tma = false;               // column tiles by TMA (needs a 16-byte multiple row pitch: not complex64 with odd N)
+    void *gen_tw = nullptr, *gen_blu_w = nullptr, *gen_blu_b = nullptr;
     CUtensorMap tmap{};                  // tensor map of the wavefront last seen by the column pass
     const void *tmap_wf = nullptr;
     std::vector<MapDesc> map_descs;     // tensor maps of surface maps, by pointer
@@ -291,6 +298,119 @@ bool valid_positive(const double *v, int n)
     return true;
 }
 
+// ---- grids that are not a power of two ---------------------------------------------------------------------------
+// Radices of a length-M mixed-radix transform (16, 8, 4, 2, then 13, 11, 7, 5, 3); false if M has another prime factor.
+bool factor_radices(int M, int *radix, int *nstages)
+{
+    int n = 0;
+    auto take = [&](int r) {
+        while (M % r == 0 && n < kGenMaxStages) { radix[n++] = r; M /= r; }
+    };
+    take(16); take(8); take(4); take(2); take(13); take(11); take(7); take(5); take(3);
+    *nstages = n;
+    return M == 1;
+}
+
+int next_smooth(int m)      // smallest 7-smooth integer >= m
+{
+    for (;; ++m) {
+        int r = m;
+        for (int p : {2, 3, 5, 7})
+            while (r % p == 0) r /= p;
+        if (r == 1) return m;
+    }
+}
+
+template <typename C> fresnel_status upload_vec(void **dev, const std::vector<C> &h)
+{
+    if (cudaMalloc(dev, h.size() * sizeof(C)) != cudaSuccess) return FRESNEL_ERR_ALLOC;
+    return cudaMemcpy(*dev, h.data(), h.size() * sizeof(C), cudaMemcpyHostToDevice) == cudaSuccess ? FRESNEL_OK : FRESNEL_ERR_CUDA;
+}
+
+// Root table W_M^m, and for Bluestein the chirp w[n] = exp(-i pi n^2/N) (n^2 mod 2N in integers: exact) and the
+// length-M transform of the chirp filter conj(w)[|m|] (zero elsewhere), scaled by 1/M -- all in long double on the
+// host, rounded once.
+template <typename C> fresnel_status build_generic_tables(fresnel_plan *p, bool bluestein)
+{
+    using T = decltype(C{}.x);
+    const int N = p->N, M = p->gen_M;
+    std::vector<C> tw(M);
+    std::vector<long double> wr(M), wi(M);
+    for (int m = 0; m < M; ++m) {
+        const long double a = -2.0L * PI_L * (long double)m / (long double)M;
+        wr[m] = cosl(a); wi[m] = sinl(a);
+        tw[m].x = (T)wr[m]; tw[m].y = (T)wi[m];
+    }
+    fresnel_status st = upload_vec(&p->gen_tw, tw);
+    if (st != FRESNEL_OK || !bluestein) return st;
+    std::vector<C> w(N), bh(M);
+    std::vector<long double> br(M, 0.0L), bi(M, 0.0L);
+    for (int n = 0; n < N; ++n) {
+        const long long q = ((long long)n * n) % (2LL * N);
+        const long double a = PI_L * (long double)q / (long double)N;
+        w[n].x = (T)cosl(a); w[n].y = (T)(-sinl(a));
+        br[n] = cosl(a); bi[n] = sinl(a);                           // conj(w)[n]
+        if (n > 0) { br[M - n] = br[n]; bi[M - n] = bi[n]; }
+    }
+    // plain O(M^2) sum: a one-off of at most ~5e7 terms per plan
+    for (int k = 0; k < M; ++k) {
+        long double sr = 0.0L, si = 0.0L;
+        long long e = 0;
+        for (int m = 0; m < M; ++m) {
+            if (br[m] != 0.0L || bi[m] != 0.0L) {
+                sr += br[m] * wr[e] - bi[m] * wi[e];
+                si += br[m] * wi[e] + bi[m] * wr[e];
+            }
+            e += k;
+            if (e >= M) e -= M;
+        }
+        bh[k].x = (T)(sr / (long double)M);
+        bh[k].y = (T)(si / (long double)M);
+    }
+    st = upload_vec(&p->gen_blu_w, w);
+    if (st != FRESNEL_OK) return st;
+    return upload_vec(&p->gen_blu_b, bh);
+}
+
+// Can the shared-memory path take this grid?  Two line buffers of the transform length (N, or the Bluestein
+// convolution length) with the narrowest column tile (16 bytes) must fit one SM's shared memory.
+bool generic_supported(int N, fresnel_dtype dt)
+{
+    int radix[kGenMaxStages], ns = 0;
+    int M = N;
+    if (!factor_radices(N, radix, &ns)) {
+        M = next_smooth(2 * N - 1);
+        if (!factor_radices(M, radix, &ns)) return false;
+    }
+    const size_t es = dt == FRESNEL_C128 ? 16 : 8;
+    return 2 * gen_buffer_bytes(M, (int)(16 / es), (int)es) + 1024 <= (size_t)kGenMaxSmem;
+}
+
+// Shared memory of the generic pass: two line buffers of M x W complex + alignment slack.
+size_t gen_smem(const fresnel_plan *p, int W) { return 2 * gen_buffer_bytes(p->gen_M, W, (int)p->esize()) + 1024; }
+
+fresnel_status setup_generic(fresnel_plan *p)
+{
+    const int N = p->N;
+    bool bluestein = !factor_radices(N, p->gen_radix, &p->gen_nstages);
+    p->gen_M = N;
+    if (bluestein) {
+        p->gen_M = next_smooth(2 * N - 1);
+        if (!factor_radices(p->gen_M, p->gen_radix, &p->gen_nstages)) return FRESNEL_ERR_UNSUPPORTED;
+    }
+    // column tiles: W complex per row, at least 16 bytes (TMA minimum; also the box start alignment), 32 where two
+    // CTAs still fit an SM
+    const int es = (int)p->esize();
+    const int wmin = 16 / es, wpref = 32 / es;
+    if (gen_smem(p, wmin) > (size_t)kGenMaxSmem) return FRESNEL_ERR_UNSUPPORTED;
+    p->gen_wcol = (2 * gen_smem(p, wpref) <= (size_t)kGenMaxSmem) ? wpref : wmin;
+    p->gen_box_rows = N < 256 ? N : 256;
+    p->gen_tma = ((size_t)N * es) % 16 == 0 && std::getenv("FRESNEL_NO_TMA") == nullptr;
+    p->generic = true;
+    p->fuse = 0;
+    return p->dtype == FRESNEL_C128 ? build_generic_tables<double2>(p, bluestein) : build_generic_tables<float2>(p, bluestein);
+}
+
 // ---- TMA tensor maps -------------------------------------------------------------------------------------
 typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
                                   const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
@@ -344,10 +464,11 @@ bool make_tensor_map(fresnel_plan *p, void *wf)
     const cuuint64_t N = (cuuint64_t)p->N;
     cuuint64_t gdim[3] = {2 * N, N, (cuuint64_t)p->batch};
     cuuint64_t gstr[2] = {N * es, N * N * es};
-    cuuint32_t box[3] = {(cuuint32_t)(2 * p->tma_w), 256u, 1u};
+    cuuint32_t box[3] = {(cuuint32_t)(2 * p->tma_w), p->generic ? (cuuint32_t)p->gen_box_rows : 256u, 1u};
     cuuint32_t estr[3] = {1, 1, 1};
     const size_t row_bytes = (size_t)p->tma_w * es;
-    CUtensorMapSwizzle sw = row_bytes == 32 ? CU_TENSOR_MAP_SWIZZLE_32B
+    CUtensorMapSwizzle sw = p->generic ? CU_TENSOR_MAP_SWIZZLE_NONE
+                          : row_bytes == 32 ? CU_TENSOR_MAP_SWIZZLE_32B
                           : row_bytes == 64 ? CU_TENSOR_MAP_SWIZZLE_64B
                           : row_bytes == 128 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE;
     CUresult r = fn(&p->tmap, dbl ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, wf, gdim, gstr, box, estr,
@@ -403,9 +524,33 @@ struct PassSpec {
     double scale = 1.0;
 };
 
+template <typename T> cudaError_t run_generic(fresnel_plan *p, void *wf, const PassSpec &q)
+{
+    using C = typename cplx_of<T>::type;
+    GenArgs<T> a;
+    std::memset(&a, 0, sizeof(a));
+    const bool tma = q.col && p->gen_tma && make_tensor_map(p, wf);
+    a.wf = (C *)wf; a.N = p->N; a.M = p->gen_M; a.W = q.col ? p->gen_wcol : 1; a.mode = q.mode;
+    a.col = q.col ? (tma ? 1 : 2) : 0;
+    a.box_rows = p->gen_box_rows;
+    a.nstages = p->gen_nstages;
+    for (int i = 0; i < p->gen_nstages; ++i) a.radix[i] = p->gen_radix[i];
+    a.tw = (const C *)p->gen_tw; a.blu_w = (const C *)p->gen_blu_w; a.blu_b = (const C *)p->gen_blu_b;
+    a.pre = (const C *)q.pre; a.mid = (const C *)q.mid; a.rowfac = (const C *)q.rowfac;
+    a.amp = (const T *)q.amp; a.opd = (const T *)q.opd; a.inv_lambda = q.inv_lambda;
+    a.scale = (T)q.scale; a.pdl = p->pdl;
+    return launch_gen_pass<T>(a, p->tmap, p->batch, gen_smem(p, a.W), p->stream);
+}
+
 fresnel_status run_pass(fresnel_plan *p, void *wf, const PassSpec &q)
 {
     cudaError_t e = cudaErrorInvalidValue;
+    if (p->generic) {
+        e = p->dtype == FRESNEL_C128 ? run_generic<double>(p, wf, q) : run_generic<float>(p, wf, q);
+        if (e != cudaSuccess) return FRESNEL_ERR_CUDA;
+        ++p->launches;
+        return FRESNEL_OK;
+    }
     const bool tma = q.col && p->tma_w > 0 && make_tensor_map(p, wf);
     const CUtensorMap *ma = &p->tmap, *mo = &p->tmap;
     if (tma && q.mode == MODE_CONV2) {
@@ -514,6 +659,16 @@ long double as_coeff(int N, double dx, double lambda, double z)
     return -(long double)lambda * (long double)z / (2.0L * nd * nd);
 }
 
+// Constant phase (turns) a centred 1-D transform of an ODD grid carries besides its two ramps: -+ (h^2 mod N)/N,
+// h = N/2, for the forward (alt = +1) / inverse (alt = -1) kernel.  Even grids: the 2-D product of the constants is 1.
+double centred_phase0(int N, int alt)
+{
+    if ((N & 1) == 0) return 0.0;
+    const long long h = N / 2;
+    const double fr = (double)((h * h) % N) / (double)N;
+    return alt > 0 ? -fr : fr;
+}
+
 std::vector<ChirpSpec> lens_key(const fresnel_plan *p, const double *pixel, const double *lambda, double f)
 {
     std::vector<ChirpSpec> key(p->batch);
@@ -576,13 +731,14 @@ fresnel_status direct_impl(fresnel_plan *p, void *wf, double *pixel_inout, const
         kin[b] = make_spec(cin, 1.0, 0.0);
         // per-axis share of dx^2/(i lambda z): dx/sqrt(lambda |z|) * exp(-+ i pi/4)
         const double a1 = (double)((long double)dx / sqrtl((long double)lambda[b] * fabsl((long double)z)));
-        kout[b] = make_spec(qpf_coeff(dx_out[b], lambda[b], z), a1, z > 0 ? -0.125 : 0.125);
+        kout[b] = make_spec(qpf_coeff(dx_out[b], lambda[b], z), a1, (z > 0 ? -0.125 : 0.125) + centred_phase0(p->N, z > 0 ? +1 : -1));
     }
-    // the (-1)^n of the centred transform rides on both tables
+    // the (-1)^n (odd N: the phase ramp) of the centred transform rides on both tables
     TableRequest r[3];
     int nreq = 2;
-    r[0] = request_table(p, KIND_CENTRED, 1, kin, cap);
-    r[1] = request_table(p, KIND_CENTRED, 1, kout, cap);
+    const int alt = z > 0 ? +1 : -1;
+    r[0] = request_table(p, KIND_CENTRED, alt, kin, cap);
+    r[1] = request_table(p, KIND_CENTRED, alt, kout, cap);
     if (opd) r[nreq++] = request_inv_lambda(p, lambda, cap);
     fresnel_status st = flush_builds(p, r, nreq);
     if (st != FRESNEL_OK) return st;
@@ -670,7 +826,8 @@ fresnel_status fresnel_plan_create(fresnel_plan **out, int N, int batch, fresnel
 {
     if (!out || batch <= 0 || N <= 0) return FRESNEL_ERR_INVALID_ARG;
     if (dtype != FRESNEL_C64 && dtype != FRESNEL_C128) return FRESNEL_ERR_UNSUPPORTED;
-    if (!is_pow2(N) || N < 64 || N > 8192) return FRESNEL_ERR_UNSUPPORTED;
+    if (N < 16 || N > 8192 || (is_pow2(N) && N < 64)) return FRESNEL_ERR_UNSUPPORTED;
+    if (!is_pow2(N) && !generic_supported(N, dtype)) return FRESNEL_ERR_UNSUPPORTED;
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev <= 0) { cudaGetLastError(); return FRESNEL_ERR_CUDA; }
     fresnel_plan *p = new (std::nothrow) fresnel_plan();
@@ -686,10 +843,16 @@ fresnel_status fresnel_plan_create(fresnel_plan **out, int N, int batch, fresnel
     }
     { const char *pd = std::getenv("FRESNEL_PDL"); p->pdl = pd ? std::atoi(pd) : 1; }
     { const char *fu = std::getenv("FRESNEL_FUSE"); p->fuse = fu ? std::atoi(fu) : 1; }
-    p->tma_w = std::getenv("FRESNEL_NO_TMA") ? 0 : query_tma_width(N, dtype);     // env switch: A/B timing only
-    p->map_box = query_map_box(N, dtype);
     p->map_descs.reserve(kMaxMapDescs);                            // pointers into it are handed out
-    fresnel_status st = upload_twiddles(p);
+    fresnel_status st;
+    if (is_pow2(N)) {
+        p->tma_w = std::getenv("FRESNEL_NO_TMA") ? 0 : query_tma_width(N, dtype);     // env switch: A/B timing only
+        p->map_box = query_map_box(N, dtype);
+        st = upload_twiddles(p);
+    } else {
+        st = setup_generic(p);                                     // mixed radix / Bluestein (gen_kernel.cuh)
+        p->tma_w = p->gen_wcol;
+    }
     if (st == FRESNEL_OK && cudaEventCreateWithFlags(&p->order_ev, cudaEventDisableTiming) != cudaSuccess) st = FRESNEL_ERR_CUDA;
     if (st == FRESNEL_OK) st = grow_slots(p, kDefaultSlots);
     if (st != FRESNEL_OK) { cudaGetLastError(); fresnel_plan_destroy(p); return st; }
@@ -751,6 +914,9 @@ fresnel_status fresnel_plan_destroy(fresnel_plan *p)
         DeviceGuard g(p);
         cudaStreamSynchronize(p->stream);
         cudaFree(p->tw);
+        cudaFree(p->gen_tw);
+        cudaFree(p->gen_blu_w);
+        cudaFree(p->gen_blu_b);
         for (void *a : p->arenas) cudaFree(a);
         if (p->order_ev) cudaEventDestroy(p->order_ev);
         cudaGetLastError();
@@ -856,11 +1022,13 @@ fresnel_status fresnel_fft2d(fresnel_plan *p, void *wf, int direction, int cente
         return run_two_passes(p, mode, wf, nullptr, nullptr, nullptr, nullptr, nullptr, per_pass);
     }
     // centred transform = s * fft2(s * u), s = (-1)^(j+k): sign tables on load and after the transform
+    // (odd N: phase ramps exp(+-2 pi i h n/N), h = N/2, and the constant exp(-+2 pi i h^2/N) per dimension)
     const CaptureState cap = capture_state(p);
-    std::vector<ChirpSpec> k1(p->batch, make_spec(0.0L, 1.0, 0.0)), k2(p->batch, make_spec(0.0L, per_pass, 0.0));
+    const int alt = mode == MODE_FWD ? +1 : -1;
+    std::vector<ChirpSpec> k1(p->batch, make_spec(0.0L, 1.0, 0.0)), k2(p->batch, make_spec(0.0L, per_pass, centred_phase0(p->N, alt)));
     TableRequest r[2];
-    r[0] = request_table(p, KIND_CENTRED, 1, k1, cap);
-    r[1] = request_table(p, KIND_CENTRED, 1, k2, cap);
+    r[0] = request_table(p, KIND_CENTRED, alt, k1, cap);
+    r[1] = request_table(p, KIND_CENTRED, alt, k2, cap);
     fresnel_status st = flush_builds(p, r, 2);
     if (st != FRESNEL_OK) return st;
     return run_two_passes(p, mode, wf, p->slots[r[0].slot].dev, p->slots[r[1].slot].dev, nullptr, nullptr, nullptr, 1.0);

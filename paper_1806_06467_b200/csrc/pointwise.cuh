@@ -58,14 +58,18 @@ __global__ void __launch_bounds__(256) intensity_kernel(const typename cplx_of<T
     using C = typename cplx_of<T>::type;
     const size_t stride = (size_t)gridDim.x * blockDim.x * 2;
     for (size_t i = ((size_t)blockIdx.x * blockDim.x + threadIdx.x) * 2; i < plane; i += stride) {
-        double a0 = (double)image[i], a1 = (double)image[i + 1];
+        const bool two = i + 1 < plane;                 // an odd grid has an odd number of pixels
+        double a0 = (double)image[i], a1 = two ? (double)image[i + 1] : 0.0;
         for (int b = 0; b < nb; ++b) {
-            const C u0 = wf[(size_t)b * plane + i], u1 = wf[(size_t)b * plane + i + 1];
+            const C u0 = wf[(size_t)b * plane + i];
             a0 = fma(wt.w[b], (double)u0.x * (double)u0.x + (double)u0.y * (double)u0.y, a0);
-            a1 = fma(wt.w[b], (double)u1.x * (double)u1.x + (double)u1.y * (double)u1.y, a1);
+            if (two) {
+                const C u1 = wf[(size_t)b * plane + i + 1];
+                a1 = fma(wt.w[b], (double)u1.x * (double)u1.x + (double)u1.y * (double)u1.y, a1);
+            }
         }
         image[i] = (T)a0;
-        image[i + 1] = (T)a1;
+        if (two) image[i + 1] = (T)a1;
     }
 }
 
@@ -78,7 +82,7 @@ cudaError_t launch_intensity(const typename cplx_of<T>::type *wf, T *image, cons
         IntensityWeights wt;
         const int nb = batch - b0 < kIntensityMaxBatch ? batch - b0 : kIntensityMaxBatch;
         for (int b = 0; b < nb; ++b) wt.w[b] = weight[b0 + b];
-        const size_t want = (plane / 2 + 255) / 256;
+        const size_t want = ((plane + 1) / 2 + 255) / 256;
         const int grid = (int)(want < (size_t)sms * 8 ? want : (size_t)sms * 8);
         intensity_kernel<T><<<grid, 256, 0, stream>>>(wf + (size_t)b0 * plane, image, wt, nb, plane);
         cudaError_t e = cudaGetLastError();

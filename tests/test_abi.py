@@ -42,7 +42,8 @@ def test_plan_create_argument_checks_and_no_cpu_fallback(binding):
     import torch
     L = binding.lib()
     h = ctypes.c_void_p()
-    assert L.fresnel_plan_create(ctypes.byref(h), 2800, 1, 1) == 2      # non power of two: UNSUPPORTED
+    assert L.fresnel_plan_create(ctypes.byref(h), 7919, 1, 1) == 2      # a prime above the Bluestein capacity: UNSUPPORTED
+    assert L.fresnel_plan_create(ctypes.byref(h), 12, 1, 1) == 2
     assert L.fresnel_plan_create(ctypes.byref(h), 16384, 1, 1) == 2
     assert L.fresnel_plan_create(ctypes.byref(h), 256, -1, 1) == 1
     assert L.fresnel_plan_create(ctypes.byref(h), 256, 1, 7) == 2

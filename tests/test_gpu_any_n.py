@@ -1,0 +1,147 @@
+"""Grids that are not a power of two ("N = 2800 ran faster than
+4096"; :259 npix = 1025), run with -m gpu.  The CUDA path (gen_kernel.cuh: mixed-radix Stockham stages in shared
+memory, Bluestein for sizes with a large prime factor) against the oracle's plain O(N^3) separable DFT, whole field,
+north-star tolerances + the max-abs bound.  Sizes: 100 = 2^2 5^2, 130 = 2 5 13, 175 = 5^2 7 (odd), 243 = 3^5 (odd),
+360 = 2^3 3^2 5, 1025 = 5^2 41 (odd, Bluestein over M = 2058), 1100 = 2^2 5^2 11, 2800 = 2^4 5^2 7.
+"""
+import math
+
+import numpy as np
+import pytest
+
+from test_gpu_parity import TOL, assert_parity, field, map_dev, map_host, to_dev
+
+pytestmark = pytest.mark.gpu
+
+SIZES = [100, 130, 175, 243, 360, 1025]
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    return torch
+
+
+@pytest.fixture(scope="module")
+def B(torch_cuda):
+    from paper_1806_06467_b200 import binding
+    binding.lib()
+    return binding
+
+
+@pytest.mark.parametrize("dtype", ["c128", "c64"])
+@pytest.mark.parametrize("N", SIZES)
+@pytest.mark.parametrize("direction,centered", [(+1, False), (-1, False), (+1, True), (-1, True)])
+def test_fft2d_any_n(torch_cuda, B, oracle, N, dtype, direction, centered):
+    """fresnel_fft2d: forward / inverse, centred (phase ramps instead of (-1)^n for odd N) / uncentred; two batch elements."""
+    u = field(N, 11000 + N, 2, dtype)
+    plan = B.Plan(N, 2, dtype)
+    d = to_dev(torch_cuda, u, dtype)
+    plan.fft2d(d, direction, centered)
+    want = np.stack([oracle.fft2d(u[b], direction, centered) for b in range(2)])
+    assert_parity(d.cpu().numpy(), want, dtype)
+
+
+@pytest.mark.parametrize("dtype", ["c128", "c64"])
+@pytest.mark.parametrize("N", SIZES)
+def test_propagate_as_and_direct_any_n(torch_cuda, B, oracle, N, dtype):
+    """Angular spectrum (FFT-order frequencies of an odd grid) and direct Fresnel with z > 0 and z < 0, per-batch
+    wavelength and pitch."""
+    u = field(N, 11100 + N, 2, dtype)
+    dx, lam = np.array([1e-5, 1.3e-5]), np.array([1e-6, 0.7e-6])
+    zc = N * dx[0] ** 2 / lam[0]
+    plan = B.Plan(N, 2, dtype)
+    d = to_dev(torch_cuda, u, dtype)
+    plan.propagate_as(d, dx, lam, 0.3 * zc)
+    want = oracle.propagate_as_batch(u, dx, lam, 0.3 * zc)
+    assert_parity(d.cpu().numpy(), want, dtype)
+    for z in (1.4 * zc, -0.9 * zc):
+        d = to_dev(torch_cuda, u, dtype)
+        px = plan.propagate_direct(d, dx, lam, z)
+        w = []
+        for b in range(2):
+            f, dxo = oracle.propagate_direct(u[b], dx[b], lam[b], z)
+            assert px[b] == pytest.approx(dxo, rel=1e-15)
+            w.append(f)
+        assert_parity(d.cpu().numpy(), np.stack(w), dtype, f"direct z={z:.3g}")
+
+
+@pytest.mark.parametrize("dtype", ["c128", "c64"])
+@pytest.mark.parametrize("N", [175, 360, 1025])
+def test_surface_and_train_any_n(torch_cuda, B, oracle, N, dtype):
+    """The fused surface (lens + amplitude + OPD + angular spectrum), the stand-alone operators, the broadband image
+    and a train with AUTO (a mix of angular spectrum and direct) on non-power-of-two grids."""
+    from paper_1806_06467_b200 import inputs
+    from paper_1806_06467_b200.inputs import Surface
+    u = field(N, 11200 + N, 2, dtype)
+    dx, lam = np.array([2e-5, 2e-5]), np.array([0.9e-6, 0.8e-6])
+    zc = N * dx[0] ** 2 / lam[0]
+    amp = inputs.circular_aperture(N, N / 3)
+    opd = inputs.psd_map(N, 2e-5, 3.0, 15e-9, 11201)
+    da, do = map_dev(torch_cuda, amp, dtype), map_dev(torch_cuda, opd, dtype)
+    plan = B.Plan(N, 2, dtype)
+    d = to_dev(torch_cuda, u, dtype)
+    plan.surface_as(d, dx, lam, 0.8, da, do, 0.25 * zc)
+    want = oracle.surface_as_batch(u, dx, lam, 0.8, map_host(amp, dtype), map_host(opd, dtype), 0.25 * zc)
+    assert_parity(d.cpu().numpy(), want, dtype)
+    # stand-alone operators
+    d = to_dev(torch_cuda, u, dtype)
+    plan.apply_qpf(d, dx, lam, -0.5)
+    plan.apply_mask(d, da, do, lam)
+    want = np.stack([oracle.apply_mask(oracle.apply_qpf(u[b], dx[b], lam[b], -0.5), map_host(amp, dtype), map_host(opd, dtype), lam[b])
+                     for b in range(2)])
+    assert_parity(d.cpu().numpy(), want, dtype)
+    # broadband image of an odd number of pixels
+    img = map_dev(torch_cuda, np.zeros((N, N)), dtype)
+    plan.accumulate_intensity(d, [0.4, 0.6], img)
+    wimg = oracle.broadband_image(want, [0.4, 0.6])
+    got = img.cpu().numpy().astype(np.float64)
+    assert np.linalg.norm(got - wimg) / np.linalg.norm(wimg) <= (1e-11 if dtype == "c128" else 2e-5)
+    # train, AUTO rule
+    surfs = [Surface(0.6, 0.4 * zc, amp, opd), Surface(-0.9, 1.7 * zc, None, opd), Surface(math.inf, 0.0, amp, None),
+             Surface(0.8, 0.3 * zc)]
+    maps = [(map_dev(torch_cuda, s.amp, dtype), map_dev(torch_cuda, s.opd, dtype)) for s in surfs]
+    d = to_dev(torch_cuda, u, dtype)
+    px, used = plan.system_run(d, dx, lam, surfs, maps=maps)
+    assert used[:3] == [0, 1, -1]
+    got = d.cpu().numpy().reshape(2, N, N)
+    hs = [Surface(s.f, s.z, map_host(s.amp, dtype), map_host(s.opd, dtype)) for s in surfs]
+    for b in range(2):
+        w, dxo, used_o = oracle.system_run(u[b], dx[b], lam[b], hs)
+        assert used_o == used and px[b] == pytest.approx(dxo, rel=1e-14)
+        assert_parity(got[b][None], w[None], dtype, f"train, wavelength {b}")
+
+
+@pytest.mark.parametrize("dtype", ["c128", "c64"])
+def test_n2800_the_papers_size(torch_cuda, B, oracle, dtype):
+    """N = 2800 = 2^4 5^2 7: one angular-spectrum step of a config-4 style random field and one
+    direct step, whole field against the oracle's O(N^3) DFT (tens of seconds of host time)."""
+    N = 2800
+    u = field(N, 11300, 1, dtype)
+    dx, lam = np.array([1e-5]), np.array([1e-6])
+    plan = B.Plan(N, 1, dtype)
+    d = to_dev(torch_cuda, u, dtype)
+    plan.propagate_as(d, dx, lam, 0.1)
+    want = oracle.propagate_as(u[0], dx[0], lam[0], 0.1)
+    assert_parity(d.cpu().numpy(), want[None], dtype)
+    d = to_dev(torch_cuda, u, dtype)
+    px = plan.propagate_direct(d, dx, lam, 0.5)
+    want, dxo = oracle.propagate_direct(u[0], dx[0], lam[0], 0.5)
+    assert px[0] == pytest.approx(dxo, rel=1e-15)
+    assert_parity(d.cpu().numpy(), want[None], dtype)
+
+
+def test_n1100_radix_11_and_capacity_limits(torch_cuda, B, oracle):
+    """1100 = 2^2 5^2 11 exercises the radix-11 butterfly; sizes beyond the shared-memory capacity are refused."""
+    import ctypes
+    N = 1100
+    u = field(N, 11400, 1, "c128")
+    plan = B.Plan(N, 1, "c128")
+    d = to_dev(torch_cuda, u, "c128")
+    plan.fft2d(d, +1, False)
+    assert_parity(d.cpu().numpy(), oracle.fft2d(u[0], +1, False)[None], "c128")
+    h = ctypes.c_void_p()
+    assert B.lib().fresnel_plan_create(ctypes.byref(h), 4100, 1, 1) == 2       # 2^2 5^2 41: Bluestein would need M >= 8199
+    assert B.lib().fresnel_plan_create(ctypes.byref(h), 7300, 1, 1) == 2

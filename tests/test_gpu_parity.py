@@ -436,7 +436,8 @@ def test_error_codes(torch_cuda, B):
     import ctypes
     L = B.lib()
     h = ctypes.c_void_p()
-    assert L.fresnel_plan_create(ctypes.byref(h), 2800, 1, 1) == 2          # UNSUPPORTED (g12)
+    assert L.fresnel_plan_create(ctypes.byref(h), 7919, 1, 1) == 2          # UNSUPPORTED: a prime above the Bluestein capacity
+    assert L.fresnel_plan_create(ctypes.byref(h), 7300, 1, 1) == 2          # smooth, but two line buffers exceed shared memory
     assert L.fresnel_plan_create(ctypes.byref(h), 32, 1, 1) == 2
     assert L.fresnel_plan_create(ctypes.byref(h), 256, 0, 1) == 1           # INVALID_ARG
     assert L.fresnel_plan_create(None, 256, 1, 1) == 1

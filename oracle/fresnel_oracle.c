@@ -28,7 +28,7 @@
  * ran N = 2800; App. B gives npix = 1025, :259) through the plain separable
  * O(N^3) DFT of item 2b -- no FFT cleverness for those.
  *
- * Parity pins: every function here is pinned in tests/test_oracle_pins.py (P0..P19 of
+ * Parity pins: every function here is pinned in tests/test_oracle_pins.py (P0..P23 of
  * DESIGN.md) against closed forms / exact identities / brute force.  Nothing is
  * "parity unpinned".
  */
@@ -489,5 +489,148 @@ int oracle_system_run(double *u, int N, double *dx_inout, double lambda, int nsu
         if (rc != ORACLE_OK) return rc;
         if (used) used[s] = m;
     }
+    return ORACLE_OK;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * Gaussian pilot-beam propagation ("following the methods in Ref. [6,
+ * Equation 82-89]" -- Lawrence 1992, which the paper does not print; the conventions below are DESIGN.md's
+ * reading g21, restated from textbook Gaussian-beam optics).
+ *
+ * A Gaussian "pilot" beam rides along with the wavefront: waist radius w0 at position zw (so zR = pi w0^2/lambda),
+ * current position z; complex beam parameter q = (z - zw) + i zR, 1/q = 1/R - i lambda/(pi w^2).  It decides on what
+ * REFERENCE SURFACE the array is kept: within rf*zR of the pilot waist a plane, outside it a sphere centred on the
+ * pilot waist, radius Rref = z - zw.  The stored array is the true field with the reference curvature removed,
+ *     U_true = U_stored * exp(i pi r^2 / (lambda Rref))          (planar: 1/Rref = 0),
+ * so the quadratic phases that are hard to sample far from focus are never put on the grid.  Propagators:
+ *   PTP(dz)  plane -> plane: angular spectrum (item 5), pixel pitch kept;
+ *   WTS(dz)  waist (plane) -> sphere of radius dz: direct Fresnel (item 6) WITHOUT its output chirp,
+ *                U_stored' = dx^2/(i lambda dz) * CFT(Q_dx(dz) U),   dx' = lambda |dz| / (N dx);
+ *   STW(dz)  sphere of radius -dz -> waist (plane): direct Fresnel WITHOUT its input chirp (it cancels the
+ *                reference curvature exactly),  U' = dx^2/(i lambda dz) * Q_dx'(dz) * CFT(U_stored).
+ * A propagation from z1 to z2 = z1 + dz:  inside->inside PTP(dz);  inside->outside PTP(zw - z1) then WTS(z2 - zw);
+ * outside->inside STW(zw - z1) then PTP(z2 - zw);  outside->outside STW(zw - z1) then WTS(z2 - zw)   (a leg of zero
+ * length is skipped).  "inside" means |z - zw| < rf * zR.
+ * A thin lens f at z multiplies the TRUE field by exp(-i pi r^2/(lambda f)) (g2) and maps the pilot beam by the ABCD
+ * rule 1/q' = 1/q - 1/f:  zw' = z - Re q', zR' = Im q', w0' = sqrt(lambda zR'/pi); the new reference is planar if
+ * |z - zw'| < rf zR', else the sphere Rref' = z - zw'.  The stored array takes the residual chirp
+ *     U_stored' = U_stored * exp(i pi r^2/lambda * (1/Rref - 1/f - 1/Rref')).
+ * Masks multiply the stored array (they do not touch the reference).
+ *
+ * state[0..4] = {w0, zw, z, Rref (INFINITY when planar), unused}; dx_inout as elsewhere.  One wavefront.
+ * legs_used (optional, 2 ints per surface): 0 none, 1 PTP, 2 WTS, 3 STW for the two legs of each propagation.
+ * ------------------------------------------------------------------------------------------ */
+static int centred_transform(double *u, int N, int forward_kernel)
+{
+    int rc;
+    if ((rc = oracle_ifftshift(u, N)) != ORACLE_OK) return rc;
+    if ((rc = fft2_core(u, N, forward_kernel ? -1 : +1, 0)) != ORACLE_OK) return rc;
+    return oracle_fftshift(u, N);
+}
+
+static void scale_minus_i_g(double *u, int N, double g)      /* u *= -i*g  =  dx^2/(i lambda dz) with g = dx^2/(lambda dz) */
+{
+#pragma omp parallel for num_threads(nthreads()) schedule(static)
+    for (long i = 0; i < (long)N * N; ++i) {
+        double re = u[2 * i + 1] * g, im = -u[2 * i] * g;
+        u[2 * i] = re; u[2 * i + 1] = im;
+    }
+}
+
+/* waist -> spherical: chirp, centred transform, scale; no output chirp */
+int oracle_wts(double *u, int N, double *dx_inout, double lambda, double dz)
+{
+    if (!u || !dx_inout || N <= 0 || !(*dx_inout > 0) || !(lambda > 0) || !isfinite(dz) || dz == 0.0) return ORACLE_ERR_INVALID_ARG;
+    const double dx = *dx_inout;
+    int rc;
+    if ((rc = oracle_apply_qpf(u, N, dx, lambda, dz)) != ORACLE_OK) return rc;
+    if ((rc = centred_transform(u, N, dz > 0)) != ORACLE_OK) return rc;
+    scale_minus_i_g(u, N, (double)((long double)dx * (long double)dx / ((long double)lambda * (long double)dz)));
+    *dx_inout = (double)((long double)lambda * fabsl((long double)dz) / ((long double)N * (long double)dx));
+    return ORACLE_OK;
+}
+
+/* spherical -> waist: centred transform, scale, output chirp at the new pitch; no input chirp */
+int oracle_stw(double *u, int N, double *dx_inout, double lambda, double dz)
+{
+    if (!u || !dx_inout || N <= 0 || !(*dx_inout > 0) || !(lambda > 0) || !isfinite(dz) || dz == 0.0) return ORACLE_ERR_INVALID_ARG;
+    const double dx = *dx_inout;
+    int rc;
+    if ((rc = centred_transform(u, N, dz > 0)) != ORACLE_OK) return rc;
+    scale_minus_i_g(u, N, (double)((long double)dx * (long double)dx / ((long double)lambda * (long double)dz)));
+    const double dx_out = (double)((long double)lambda * fabsl((long double)dz) / ((long double)N * (long double)dx));
+    if ((rc = oracle_apply_qpf(u, N, dx_out, lambda, dz)) != ORACLE_OK) return rc;
+    *dx_inout = dx_out;
+    return ORACLE_OK;
+}
+
+/* u *= exp(i pi r^2 kappa / lambda), kappa in 1/m (a QPF with 1/z = kappa); kappa == 0: nothing */
+static int apply_curvature(double *u, int N, double dx, double lambda, long double kappa)
+{
+    if (kappa == 0.0L) return ORACLE_OK;
+    return oracle_apply_qpf(u, N, dx, lambda, (double)(1.0L / kappa));
+}
+
+int oracle_system_run_pilot(double *u, int N, double *dx_inout, double lambda, int nsurf, const double *f,
+                            const double *const *amp, const double *const *opd, const double *z,
+                            double rayleigh_factor, double *state, int *legs_used)
+{
+    if (!u || !dx_inout || !state || nsurf < 0 || (nsurf > 0 && (!f || !z))) return ORACLE_ERR_INVALID_ARG;
+    if (!(state[0] > 0) || !(rayleigh_factor > 0) || !(lambda > 0) || !(*dx_inout > 0)) return ORACLE_ERR_INVALID_ARG;
+    long double w0 = state[0], zw = state[1], zc = state[2];
+    long double inv_rref = isfinite(state[3]) ? 1.0L / (long double)state[3] : 0.0L;
+    const long double rf = rayleigh_factor, lam = lambda;
+    int rc;
+    for (int s = 0; s < nsurf; ++s) {
+        if (isnan(f[s]) || f[s] == 0.0 || !isfinite(z[s])) return ORACLE_ERR_INVALID_ARG;
+        /* (1) thin lens: ABCD on the pilot beam, residual chirp on the array */
+        if (isfinite(f[s])) {
+            const long double zR = PI_L * w0 * w0 / lam;
+            const long double qr = zc - zw, qi = zR;                 /* q = qr + i qi */
+            const long double den = qr * qr + qi * qi;
+            const long double ir = qr / den - 1.0L / (long double)f[s], ii = -qi / den;   /* 1/q' */
+            const long double d2 = ir * ir + ii * ii;
+            const long double q2r = ir / d2, q2i = -ii / d2;          /* q' */
+            const long double zw2 = zc - q2r, zR2 = q2i;
+            const long double inv_rref2 = (fabsl(zc - zw2) < rf * zR2) ? 0.0L : 1.0L / (zc - zw2);
+            const long double kappa = inv_rref - 1.0L / (long double)f[s] - inv_rref2;
+            if ((rc = apply_curvature(u, N, *dx_inout, lambda, kappa)) != ORACLE_OK) return rc;
+            zw = zw2;
+            w0 = sqrtl(lam * zR2 / PI_L);
+            inv_rref = inv_rref2;
+        }
+        /* (2) optic phasor on the stored array */
+        const double *a = amp ? amp[s] : NULL, *o = opd ? opd[s] : NULL;
+        if ((a || o) && (rc = oracle_apply_mask(u, N, a, o, lambda)) != ORACLE_OK) return rc;
+        /* (3) propagation by z[s] */
+        int leg[2] = {0, 0};
+        if (z[s] != 0.0) {
+            const long double zR = PI_L * w0 * w0 / lam;
+            const long double z1 = zc, z2 = zc + (long double)z[s];
+            const int in1 = inv_rref == 0.0L;                          /* the reference says where we are */
+            const int in2 = fabsl(z2 - zw) < rf * zR;
+            if (in1 && in2) {
+                if ((rc = oracle_propagate_as(u, N, *dx_inout, lambda, z[s])) != ORACLE_OK) return rc;
+                leg[0] = 1;
+            } else {
+                const double d1 = (double)(zw - z1), d2 = (double)(z2 - zw);
+                if (d1 != 0.0) {
+                    if (in1) { rc = oracle_propagate_as(u, N, *dx_inout, lambda, d1); leg[0] = 1; }
+                    else     { rc = oracle_stw(u, N, dx_inout, lambda, d1); leg[0] = 3; }
+                    if (rc != ORACLE_OK) return rc;
+                }
+                if (d2 != 0.0) {
+                    if (in2) { rc = oracle_propagate_as(u, N, *dx_inout, lambda, d2); leg[1] = 1; }
+                    else     { rc = oracle_wts(u, N, dx_inout, lambda, d2); leg[1] = 2; }
+                    if (rc != ORACLE_OK) return rc;
+                }
+            }
+            zc = z2;
+            inv_rref = in2 ? 0.0L : 1.0L / (z2 - zw);
+        }
+        if (legs_used) { legs_used[2 * s] = leg[0]; legs_used[2 * s + 1] = leg[1]; }
+    }
+    state[0] = (double)w0; state[1] = (double)zw; state[2] = (double)zc;
+    state[3] = inv_rref == 0.0L ? INFINITY : (double)(1.0L / inv_rref);
     return ORACLE_OK;
 }

@@ -48,6 +48,13 @@ def lib():
         L.oracle_system_run.argtypes = [dp, ctypes.c_int, dp, ctypes.c_double, ctypes.c_int, dp, pp, pp, dp,
                                         ctypes.POINTER(ctypes.c_int), ctypes.POINTER(ctypes.c_int)]
         L.oracle_system_run.restype = ctypes.c_int
+        L.oracle_wts.argtypes = [dp, ctypes.c_int, dp, ctypes.c_double, ctypes.c_double]
+        L.oracle_wts.restype = ctypes.c_int
+        L.oracle_stw.argtypes = [dp, ctypes.c_int, dp, ctypes.c_double, ctypes.c_double]
+        L.oracle_stw.restype = ctypes.c_int
+        L.oracle_system_run_pilot.argtypes = [dp, ctypes.c_int, dp, ctypes.c_double, ctypes.c_int, dp, pp, pp, dp,
+                                              ctypes.c_double, dp, ctypes.POINTER(ctypes.c_int)]
+        L.oracle_system_run_pilot.restype = ctypes.c_int
         L.oracle_accumulate_intensity.argtypes = [dp, ctypes.c_int, ctypes.c_double, dp]
         L.oracle_accumulate_intensity.restype = ctypes.c_int
         for name in ("oracle_dft2_naive", "oracle_fft2", "oracle_fftshift", "oracle_ifftshift", "oracle_fft2d",
@@ -228,3 +235,47 @@ def system_run(u, dx, lam, surfaces, methods=None):
                                    z.ctypes.data_as(dp), m.ctypes.data_as(ctypes.POINTER(ctypes.c_int)),
                                    used.ctypes.data_as(ctypes.POINTER(ctypes.c_int))), "system_run")
     return a, dxv.value, [int(x) for x in used[:n]]
+
+
+def wts(u, dx, lam, dz):
+    """Waist -> spherical (direct Fresnel without its output chirp).  Returns (stored field, dx_out)."""
+    a, N = _prep(u)
+    d = ctypes.c_double(float(dx))
+    _check(lib().oracle_wts(_dptr(a), N, ctypes.byref(d), float(lam), float(dz)), "wts")
+    return a, d.value
+
+
+def stw(u, dx, lam, dz):
+    """Spherical -> waist (direct Fresnel without its input chirp).  Returns (field, dx_out)."""
+    a, N = _prep(u)
+    d = ctypes.c_double(float(dx))
+    _check(lib().oracle_stw(_dptr(a), N, ctypes.byref(d), float(lam), float(dz)), "stw")
+    return a, d.value
+
+
+LEG_NONE, LEG_PTP, LEG_WTS, LEG_STW = 0, 1, 2, 3
+
+
+def system_run_pilot(u, dx, lam, surfaces, w0, rayleigh_factor=1.0, state=None):
+    """Train of surfaces under the Gaussian pilot-beam rule (NEXT-1; conventions in fresnel_oracle.c).  `state`:
+    (w0, zw, z, Rref) to continue from, default a waist of radius w0 at z = 0 on a planar reference.
+    Returns (stored field, final pixel pitch, state tuple (w0, zw, z, Rref), legs [(leg1, leg2), ...])."""
+    a, N = _prep(u)
+    n = len(surfaces)
+    dp = ctypes.POINTER(ctypes.c_double)
+    f = np.array([math.inf if s.f is None else float(s.f) for s in surfaces], dtype=np.float64)
+    z = np.array([float(s.z) for s in surfaces], dtype=np.float64)
+    keep, amp_p, opd_p = [], (dp * max(n, 1))(), (dp * max(n, 1))()
+    for i, s in enumerate(surfaces):
+        ka, pa = _real(s.amp, N)
+        ko, po = _real(s.opd, N)
+        keep += [ka, ko]
+        amp_p[i] = pa if pa is not None else ctypes.cast(None, dp)
+        opd_p[i] = po if po is not None else ctypes.cast(None, dp)
+    dxv = ctypes.c_double(float(dx))
+    st = np.array([float(w0), 0.0, 0.0, math.inf, 0.0] if state is None else list(state) + [0.0], dtype=np.float64)
+    legs = np.zeros(2 * max(n, 1), dtype=np.int32)
+    _check(lib().oracle_system_run_pilot(_dptr(a), N, ctypes.byref(dxv), float(lam), n, f.ctypes.data_as(dp), amp_p, opd_p,
+                                         z.ctypes.data_as(dp), float(rayleigh_factor), st.ctypes.data_as(dp),
+                                         legs.ctypes.data_as(ctypes.POINTER(ctypes.c_int))), "system_run_pilot")
+    return a, dxv.value, tuple(float(x) for x in st[:4]), [(int(legs[2 * i]), int(legs[2 * i + 1])) for i in range(n)]

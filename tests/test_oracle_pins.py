@@ -552,3 +552,122 @@ def test_P19_exact_identities_any_N(oracle):
         b, dxo = oracle.propagate_direct(g, 2e-5, lam, zc)
         assert dxo == pytest.approx(2e-5, rel=1e-14)
         assert rel(a, b) <= 1e-9
+
+
+# ---- P20-P23: Gaussian pilot-beam propagation (reading g21) ----
+def true_field(stored, dx, lam, rref):
+    """Put the reference-sphere curvature back: U_true = U_stored exp(i pi r^2/(lam Rref)) (planar: unchanged)."""
+    if not math.isfinite(rref):
+        return stored
+    x, y = coords(stored.shape[0], dx)
+    return stored * np.exp(1j * np.pi * (x * x + y * y) / (lam * rref))
+
+
+def test_P20_pilot_free_space_is_the_gaussian_beam(oracle):
+    """The pilot beam IS the Gaussian: start at its waist, go 0.3 zR (stays planar: one PTP leg), 8 zR (one WTS leg,
+    spherical reference of radius z) and back.  The TRUE field must equal (q0/q) exp(i pi r^2/(lam q)); the state
+    must say w0, waist at 0, position z, Rref = z; on the sphere the stored phase is flat up to the small
+    1/R(z) - 1/z mismatch, i.e. far flatter than the true field's."""
+    from paper_1806_06467_b200.inputs import Surface
+    N, dx, lam, w0 = 512, 1e-5, 1e-6, 2e-4
+    zR = math.pi * w0 * w0 / lam
+    u0 = gaussian_closed_form(N, dx, lam, w0, 0.0)
+    v, d1, st, legs = oracle.system_run_pilot(u0, dx, lam, [Surface(math.inf, 0.3 * zR)], w0)
+    assert legs == [(oracle.LEG_PTP, 0)] and d1 == dx and st == (w0, 0.0, 0.3 * zR, math.inf)
+    assert rel(v, gaussian_closed_form(N, dx, lam, w0, 0.3 * zR)) <= 1e-9
+    z = 8.0 * zR
+    v, d1, st, legs = oracle.system_run_pilot(u0, dx, lam, [Surface(math.inf, z)], w0)
+    assert legs == [(0, oracle.LEG_WTS)]
+    assert d1 == pytest.approx(lam * z / (N * dx), rel=1e-15)
+    assert st[0] == pytest.approx(w0, rel=1e-15) and st[1] == 0.0 and st[2] == pytest.approx(z) and st[3] == pytest.approx(z)
+    assert rel(true_field(v, d1, lam, st[3]), gaussian_closed_form(N, d1, lam, w0, z)) <= 1e-9
+    c = N // 2
+    w_z = w0 * math.sqrt(1 + (z / zR) ** 2)
+    k = int(round(w_z / d1))                                   # one beam radius away from the axis
+    stored_dphi = abs(np.angle(v[c, c + k] / v[c, c]))
+    true_dphi = math.pi * (k * d1) ** 2 / (lam * z * (1 + (zR / z) ** 2))
+    # residual pi w^2/lam (1/R - 1/z) = 65/8 * (1 - 64/65) = 0.125 rad at one beam radius, against 8 rad of true curvature
+    assert stored_dphi == pytest.approx(0.125, rel=0.1) and true_dphi > 7.5     # the curvature lives in the reference, not on the grid
+    # and back to the waist: one STW leg, the input returns
+    w, d2, st2, legs = oracle.system_run_pilot(v, d1, lam, [Surface(math.inf, -z)], w0, state=st)
+    assert legs == [(oracle.LEG_STW, 0)] and d2 == pytest.approx(dx, rel=1e-14) and not math.isfinite(st2[3])
+    assert rel(w, u0) <= 1e-10
+
+
+def test_P21_pilot_legs_equal_the_existing_propagators(oracle):
+    """Where they coincide the pilot-beam legs ARE the existing operators: inside the Rayleigh range the result is
+    propagate_as bit for bit (and two such steps equal one: PTP o PTP = PTP); a waist-to-sphere leg times the output
+    chirp is propagate_direct; a sphere-to-waist leg applied to a de-chirped field is propagate_direct too; crossing
+    the waist region from sphere to sphere takes STW then WTS and equals direct o direct on the true fields."""
+    from paper_1806_06467_b200.inputs import Surface
+    N, dx, lam, w0 = 256, 2e-5, 1e-6, 4e-4
+    zR = math.pi * w0 * w0 / lam                                 # 0.503 m
+    x, y = coords(N, dx)
+    u = np.exp(-(x * x + y * y) / w0 ** 2) * (1 + 0.1 * np.cos(2 * np.pi * x / 2e-4)) * np.exp(0.2j * np.sin(2 * np.pi * y / 3e-4))
+    a, d, st, legs = oracle.system_run_pilot(u, dx, lam, [Surface(math.inf, 0.2 * zR)], w0)
+    assert np.array_equal(a, oracle.propagate_as(u, dx, lam, 0.2 * zR)) and legs == [(1, 0)]
+    b, _, st2, _ = oracle.system_run_pilot(u, dx, lam, [Surface(math.inf, 0.12 * zR), Surface(math.inf, 0.08 * zR)], w0)
+    assert rel(b, a) <= 1e-13 and st2[2] == pytest.approx(0.2 * zR)
+    z = 3.0 * zR
+    s, d1, st, legs = oracle.system_run_pilot(u, dx, lam, [Surface(math.inf, z)], w0)
+    want, dxo = oracle.propagate_direct(u, dx, lam, z)
+    assert legs == [(0, 2)] and d1 == dxo
+    assert rel(true_field(s, d1, lam, st[3]), want) <= 1e-13
+    # sphere -> sphere through the waist: from z = -3 zR to +2 zR
+    st_in = (w0, 0.0, -z, -z)
+    stored_in = u                                                # any stored array will do
+    t, d2, st3, legs = oracle.system_run_pilot(stored_in, dx, lam, [Surface(math.inf, z + 2 * zR)], w0, state=st_in)
+    assert legs == [(3, 2)] and st3[3] == pytest.approx(2 * zR)
+    m, dm = oracle.propagate_direct(true_field(stored_in, dx, lam, -z), dx, lam, z)
+    m, dm = oracle.propagate_direct(m, dm, lam, 2 * zR)
+    assert d2 == pytest.approx(dm, rel=1e-14)
+    assert rel(true_field(t, d2, lam, st3[3]), m) <= 1e-12
+    # energy: sum |U|^2 dx^2 is conserved by every leg
+    assert np.sum(np.abs(t) ** 2) * d2 ** 2 == pytest.approx(np.sum(np.abs(u) ** 2) * dx ** 2, rel=1e-12)
+
+
+def test_P22_pilot_through_lenses_lands_on_the_abcd_closed_form(oracle):
+    """Config 2 (Gaussian through three lenses) under the pilot-beam rule: after every surface the TRUE field equals
+    the ABCD closed form of P5, the pilot state equals the closed-form beam (waist position and Rayleigh range from q),
+    and the first propagation -- from a lens 0.499 m before its focus to 0.9 mm past it -- is STW then PTP."""
+    from paper_1806_06467_b200 import inputs
+    wl = inputs.config2()
+    N, dx, lam, w0 = wl.N, float(wl.dx[0]), float(wl.lam[0]), 2e-3
+    steps = [(s.f, s.z) for s in wl.surfaces]
+    ref = abcd_chain(lam, w0, steps)
+    u, d, st, zpos = wl.field[0], dx, None, 0.0
+    for i, (s, (q, A)) in enumerate(zip(wl.surfaces, ref)):
+        u, d, st, legs = oracle.system_run_pilot(u, d, lam, [s], w0, state=st)
+        zpos += s.z
+        if i == 0:
+            assert legs == [(oracle.LEG_STW, oracle.LEG_PTP)]
+        x, y = coords(N, d)
+        assert rel(true_field(u, d, lam, st[3]), A * np.exp(1j * np.pi * (x * x + y * y) / (lam * q))) <= 1e-8, f"surface {i}"
+        # closed-form beam: q = (z - zw) - i zR in the sign convention of abcd_chain
+        assert st[2] == pytest.approx(zpos, rel=1e-14)
+        assert st[2] - st[1] == pytest.approx(q.real, rel=1e-9, abs=1e-12)
+        assert math.pi * st[0] ** 2 / lam == pytest.approx(-q.imag, rel=1e-9)
+    assert st[0] == pytest.approx(math.sqrt(lam * 0.333305 / math.pi), rel=1e-5)       # zR = 0.333305 m after lens 3 (SURVEY P5)
+
+
+def test_P23_pilot_masks_rayleigh_factor_and_errors(oracle):
+    """Masks act on the stored array; the Rayleigh factor moves the planar/spherical boundary; a zero-length step and a
+    z = 0 surface do nothing to the reference; bad arguments are refused."""
+    from paper_1806_06467_b200 import inputs
+    from paper_1806_06467_b200.inputs import Surface
+    N, dx, lam, w0 = 128, 2e-5, 1e-6, 3e-4
+    zR = math.pi * w0 * w0 / lam
+    u = rnd(N, 230)
+    amp = inputs.circular_aperture(N, 40)
+    opd = inputs.psd_map(N, dx, 3.0, 20e-9, 231)
+    z = 1.5 * zR
+    _, _, _, legs1 = oracle.system_run_pilot(u, dx, lam, [Surface(math.inf, z)], w0, rayleigh_factor=1.0)
+    _, _, _, legs2 = oracle.system_run_pilot(u, dx, lam, [Surface(math.inf, z)], w0, rayleigh_factor=2.0)
+    assert legs1 == [(0, 2)] and legs2 == [(1, 0)]
+    a, d, st, legs = oracle.system_run_pilot(u, dx, lam, [Surface(math.inf, 0.0, amp, opd), Surface(math.inf, z)], w0)
+    b, d2 = oracle.wts(oracle.apply_mask(u, amp, opd, lam), dx, lam, z)
+    assert legs == [(0, 0), (0, 2)] and d == d2 and np.array_equal(a, b)
+    with pytest.raises(oracle.OracleError):
+        oracle.system_run_pilot(u, dx, lam, [Surface(0.0, 0.1)], w0)
+    with pytest.raises(oracle.OracleError):
+        oracle.system_run_pilot(u, dx, lam, [Surface(math.inf, 0.1)], -1.0)

@@ -203,6 +203,37 @@ enum { FRESNEL_METHOD_AS = 0, FRESNEL_METHOD_DIRECT = 1, FRESNEL_METHOD_AUTO = 2
 fresnel_status fresnel_system_run(fresnel_plan *p, void *wf, double *pixel_inout, const double *lambda,
                                   const fresnel_surface *surf, int nsurf, int *method_used);
 
+/* A train of surfaces under the GAUSSIAN PILOT-BEAM rule ("following the methods in Ref. [6, Equation
+ * 82-89]" -- Lawrence 1992, not printed in the paper; reading g21 states every convention; SURVEY.md sec.
+ * 8(f) NEXT-1).  A Gaussian pilot beam per batch element -- waist radius w0 at position zw (zR = pi w0^2 / lambda),
+ * current position z -- decides on which reference surface the array is kept: a plane within rayleigh_factor * zR
+ * of the pilot waist, outside it a sphere centred on the waist (radius rref = z - zw) whose curvature is REMOVED
+ * from the array,   U_true = U_stored * exp(i pi r^2 / (lambda rref)),   so the quadratic phases that cannot be
+ * sampled far from focus never reach the grid.  A propagation from z1 to z2 takes
+ *     inside -> inside    PTP(z2 - z1)                          angular spectrum, pitch kept
+ *     inside -> outside   PTP(zw - z1), WTS(z2 - zw)            waist -> sphere: direct Fresnel without its output chirp
+ *     outside -> inside   STW(zw - z1), PTP(z2 - zw)            sphere -> waist: direct Fresnel without its input chirp
+ *     outside -> outside  STW(zw - z1), WTS(z2 - zw)            (a leg of zero length is skipped)
+ * each WTS / STW leg changing the pitch to lambda |dz| / (N dx).  A thin lens f maps the pilot beam by the ABCD rule
+ * 1/q' = 1/q - 1/f (q = z - zw + i zR), chooses the new reference (plane if |z - zw'| < rayleigh_factor zR', else the
+ * sphere rref' = z - zw') and leaves on the array only the residual chirp exp(i pi r^2/lambda (1/rref - 1/f - 1/rref')),
+ * which rides on the next pass.  Masks act on the stored array.  Surfaces: as in fresnel_system_run (`method` is
+ * ignored).  state: HOST array of `batch` pilot states, read as the starting state (a collimated beam of radius R at
+ * its waist: {R, 0, 0, INFINITY}) and overwritten with the final one; legs_used (HOST, 2 ints per surface, may be
+ * NULL): 0 none, 1 PTP, 2 WTS, 3 STW.  Every batch element must take the same legs (and every WTS / STW leg the same
+ * direction), otherwise FRESNEL_ERR_UNSUPPORTED; everything is validated before anything is enqueued.  The kernels
+ * are the two-pass kernels of the other calls: only the tables differ. */
+typedef struct {
+    double w0;    /* waist radius of the pilot beam (m) */
+    double zw;    /* position of its waist along the axis (m) */
+    double z;     /* current position (m) */
+    double rref;  /* radius of the reference sphere the array is stored on; +-INFINITY: planar */
+} fresnel_pilot_state;
+enum { FRESNEL_LEG_NONE = 0, FRESNEL_LEG_PTP = 1, FRESNEL_LEG_WTS = 2, FRESNEL_LEG_STW = 3 };
+fresnel_status fresnel_system_run_pilot(fresnel_plan *p, void *wf, double *pixel_inout, const double *lambda,
+                                        const fresnel_surface *surf, int nsurf, double rayleigh_factor,
+                                        fresnel_pilot_state *state, int *legs_used);
+
 /* Broadband (polychromatic) image: the incoherent, weighted sum of the batch's monochromatic intensities
  * ("calculations must be repeated for all of the wavelengths"; one process per wavelength in
  * the paper):

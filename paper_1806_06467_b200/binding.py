@@ -29,7 +29,7 @@ SYMBOLS = (
     "fresnel_plan_create", "fresnel_plan_set_stream", "fresnel_plan_synchronize", "fresnel_plan_destroy",
     "fresnel_plan_launch_count", "fresnel_plan_record_pass_events", "fresnel_plan_record_train_events",
     "fresnel_plan_last_schedule", "fresnel_plan_reserve_tables", "fresnel_plan_release_graph_tables", "fresnel_apply_qpf", "fresnel_apply_mask", "fresnel_fft2d",
-    "fresnel_propagate_as", "fresnel_propagate_direct", "fresnel_surface_as", "fresnel_system_run", "fresnel_accumulate_intensity", "fresnel_memcpy_h2d",
+    "fresnel_propagate_as", "fresnel_propagate_direct", "fresnel_surface_as", "fresnel_system_run", "fresnel_system_run_pilot", "fresnel_accumulate_intensity", "fresnel_memcpy_h2d",
     "fresnel_memcpy_d2h", "fresnel_status_string", "fresnel_version",
 )
 
@@ -41,6 +41,13 @@ METHOD_AS, METHOD_DIRECT, METHOD_AUTO = 0, 1, 2
 class _Surface(ctypes.Structure):       # fresnel_surface of include/fresnel.h
     _fields_ = [("f", ctypes.c_double), ("amp", ctypes.c_void_p), ("opd", ctypes.c_void_p),
                 ("z", ctypes.c_double), ("method", ctypes.c_int)]
+
+
+class _PilotState(ctypes.Structure):   # fresnel_pilot_state of include/fresnel.h
+    _fields_ = [("w0", ctypes.c_double), ("zw", ctypes.c_double), ("z", ctypes.c_double), ("rref", ctypes.c_double)]
+
+
+LEG_NONE, LEG_PTP, LEG_WTS, LEG_STW = 0, 1, 2, 3
 
 
 class _PassInfo(ctypes.Structure):      # fresnel_pass_info of include/fresnel.h
@@ -82,6 +89,7 @@ def lib() -> ctypes.CDLL:
     L.fresnel_propagate_direct.argtypes = [vp, vp, dp, dp, cd]
     L.fresnel_surface_as.argtypes = [vp, vp, dp, dp, cd, vp, vp, cd]
     L.fresnel_system_run.argtypes = [vp, vp, dp, dp, ctypes.POINTER(_Surface), ci, ctypes.POINTER(ci)]
+    L.fresnel_system_run_pilot.argtypes = [vp, vp, dp, dp, ctypes.POINTER(_Surface), ci, cd, ctypes.POINTER(_PilotState), ctypes.POINTER(ci)]
     L.fresnel_accumulate_intensity.argtypes = [vp, vp, dp, vp]
     L.fresnel_memcpy_h2d.argtypes = [vp, vp, vp, ctypes.c_size_t]
     L.fresnel_memcpy_d2h.argtypes = [vp, vp, vp, ctypes.c_size_t]
@@ -259,6 +267,35 @@ class Plan:
         used = (ctypes.c_int * max(n, 1))()
         self._chk(lib().fresnel_system_run(self._h, self._wf(wf), pp, lp, arr, n, used), "fresnel_system_run")
         return pa, [int(used[i]) for i in range(n)]
+
+    def system_run_pilot(self, wf, pixel, lam, surfaces, w0, maps=None, rayleigh_factor: float = 1.0, state=None):
+        """Train of surfaces under the Gaussian pilot-beam rule.  w0: pilot waist radius at the start (scalar or per
+        batch element); state: list of (w0, zw, z, rref) per batch element to continue from (default: at the waist, z = 0,
+        planar).  Returns (final pixel pitch per batch element, list of states, legs [(leg1, leg2), ...] per surface)."""
+        n = len(surfaces)
+        arr = (_Surface * max(n, 1))()
+        for i, s in enumerate(surfaces):
+            amp, opd = (maps[i] if maps is not None else (None, None))
+            arr[i].f = math.inf if s.f is None else float(s.f)
+            arr[i].amp = self._map(amp).value
+            arr[i].opd = self._map(opd).value
+            arr[i].z = float(s.z)
+            arr[i].method = METHOD_AUTO
+        pa, _ = _darr(pixel, self.batch)
+        pa = pa.copy()
+        pp = pa.ctypes.data_as(ctypes.POINTER(ctypes.c_double))
+        _, lp = _darr(lam, self.batch)
+        st = (_PilotState * self.batch)()
+        w0a, _ = _darr(w0, self.batch)
+        for b in range(self.batch):
+            if state is None:
+                st[b].w0, st[b].zw, st[b].z, st[b].rref = float(w0a[b]), 0.0, 0.0, math.inf
+            else:
+                st[b].w0, st[b].zw, st[b].z, st[b].rref = (float(x) for x in state[b])
+        legs = (ctypes.c_int * (2 * max(n, 1)))()
+        self._chk(lib().fresnel_system_run_pilot(self._h, self._wf(wf), pp, lp, arr, n, float(rayleigh_factor), st, legs),
+                  "fresnel_system_run_pilot")
+        return pa, [(st[b].w0, st[b].zw, st[b].z, st[b].rref) for b in range(self.batch)], [(int(legs[2 * i]), int(legs[2 * i + 1])) for i in range(n)]
 
     def accumulate_intensity(self, wf, weight, image) -> None:
         """image += sum_b weight[b] * |wf[b]|^2 (image: real N x N device tensor of the plan's precision)."""

@@ -669,6 +669,12 @@ double centred_phase0(int N, int alt)
     return alt > 0 ? -fr : fr;
 }
 
+// chirp exp(i pi r^2 kappa / lambda) as a table coefficient (turns per pixel^2): kappa dx^2 / (2 lambda); a thin lens is kappa = -1/f
+long double curvature_coeff(double dx, double lambda, long double kappa)
+{
+    return kappa * (long double)dx * (long double)dx / (2.0L * (long double)lambda);
+}
+
 std::vector<ChirpSpec> lens_key(const fresnel_plan *p, const double *pixel, const double *lambda, double f)
 {
     std::vector<ChirpSpec> key(p->batch);
@@ -682,20 +688,28 @@ std::vector<ChirpSpec> transfer_key(const fresnel_plan *p, const double *pixel, 
     return key;
 }
 
-// ---- one fused surface (thin lens + optic phasor + angular spectrum), two passes ------------------------------
-fresnel_status surface_as_impl(fresnel_plan *p, void *wf, const double *pixel, const double *lambda,
-                               double f, const void *amp, const void *opd, double z, int surface = -1)
+// ---- angular-spectrum leg: [chirp] -> [optic phasor] -> propagation, two passes ----------------------------------
+// chirp_key: the table of the input chirp (a thin lens, or the residual reference curvature of the pilot-beam rule),
+// empty for none; z: per batch element (all zero: optic only).
+fresnel_status as_leg(fresnel_plan *p, void *wf, const double *pixel, const double *lambda, const std::vector<ChirpSpec> &chirp_key,
+                      const void *amp, const void *opd, const double *z, int surface)
 {
     ++p->pin_epoch;
     const CaptureState cap = capture_state(p);
-    const bool lens = std::isfinite(f);
-    const bool prop = z != 0.0;
+    const bool lens = !chirp_key.empty();
+    bool prop = false;
+    for (int b = 0; b < p->batch; ++b) prop = prop || z[b] != 0.0;
     if (!lens && !prop && !amp && !opd) return FRESNEL_OK;
 
     TableRequest r[3];
     int nreq = 0, i_lens = -1, i_h = -1, i_s = -1;
-    if (lens) { i_lens = nreq; r[nreq++] = request_table(p, KIND_CENTRED, 0, lens_key(p, pixel, lambda, f), cap); }
-    if (prop) { i_h = nreq; r[nreq++] = request_table(p, KIND_FFTORDER, 0, transfer_key(p, pixel, lambda, z), cap); }
+    if (lens) { i_lens = nreq; r[nreq++] = request_table(p, KIND_CENTRED, 0, chirp_key, cap); }
+    if (prop) {
+        std::vector<ChirpSpec> key(p->batch);
+        for (int b = 0; b < p->batch; ++b) key[b] = make_spec(as_coeff(p->N, pixel[b], lambda[b], z[b]), 1.0 / (double)p->N, 0.0);
+        i_h = nreq;
+        r[nreq++] = request_table(p, KIND_FFTORDER, 0, key, cap);
+    }
     if (opd) { i_s = nreq; r[nreq++] = request_inv_lambda(p, lambda, cap); }
     fresnel_status st = flush_builds(p, r, nreq);
     if (st != FRESNEL_OK) return st;
@@ -711,43 +725,68 @@ fresnel_status surface_as_impl(fresnel_plan *p, void *wf, const double *pixel, c
     return run_two_passes(p, MODE_CONV, wf, tl, th, amp, opd, il, 1.0, surface);
 }
 
-// [thin lens f] -> [optic phasor] -> direct Fresnel propagation by z, in the two passes of the transform:
-// the lens chirp and the input chirp of the propagator are the same kind of factor, so their
-// coefficients are added (long double) and ONE table serves both; the optic phasor rides on the row-pass load.
-fresnel_status direct_impl(fresnel_plan *p, void *wf, double *pixel_inout, const double *lambda, double z,
-                           double f, const void *amp, const void *opd, int surface = -1)
+// one fused surface (thin lens + optic phasor + angular spectrum)
+fresnel_status surface_as_impl(fresnel_plan *p, void *wf, const double *pixel, const double *lambda,
+                               double f, const void *amp, const void *opd, double z, int surface = -1)
+{
+    std::vector<double> zb(p->batch, z);
+    return as_leg(p, wf, pixel, lambda, std::isfinite(f) ? lens_key(p, pixel, lambda, f) : std::vector<ChirpSpec>(), amp, opd, zb.data(), surface);
+}
+
+// ---- single-transform leg: [extra chirp] -> [optic phasor] -> centred transform with the Fresnel factors ----------
+//   FT_DIRECT  direct Fresnel: input chirp Q_dx(dz), transform, dx^2/(i lambda dz), output chirp Q_dx'(dz);
+//   FT_WTS     waist -> sphere (pilot-beam rule): no output chirp;    FT_STW   sphere -> waist: no input chirp.
+// An extra chirp on the input side (a thin lens, the residual reference curvature) is the same kind of factor as the
+// propagator's input chirp: the coefficients are added (long double) and ONE table serves both; the optic phasor
+// rides on the row-pass load.  dz, kappa: per batch element (kappa may be null); every dz must have the same sign.
+enum { FT_DIRECT = 0, FT_WTS = 1, FT_STW = 2 };
+
+fresnel_status ft_leg(fresnel_plan *p, void *wf, double *pixel_inout, const double *lambda, const double *dz, int kind,
+                      const long double *kappa, const void *amp, const void *opd, int surface)
 {
     ++p->pin_epoch;
     const CaptureState cap = capture_state(p);
-    const bool lens = std::isfinite(f);
+    const bool fwd = dz[0] > 0;
     std::vector<ChirpSpec> kin(p->batch), kout(p->batch);
     std::vector<double> dx_out(p->batch);
     for (int b = 0; b < p->batch; ++b) {
+        if ((dz[b] > 0) != fwd || dz[b] == 0.0) return FRESNEL_ERR_UNSUPPORTED;
         const double dx = pixel_inout[b];
-        const long double dxo = (long double)lambda[b] * fabsl((long double)z) / ((long double)p->N * (long double)dx);
+        const long double z = dz[b];
+        const long double dxo = (long double)lambda[b] * fabsl(z) / ((long double)p->N * (long double)dx);
         dx_out[b] = (double)dxo;
-        long double cin = qpf_coeff(dx, lambda[b], z);
-        if (lens) cin += qpf_coeff(dx, lambda[b], -(long double)f);
+        long double cin = kind != FT_STW ? qpf_coeff(dx, lambda[b], z) : 0.0L;
+        if (kappa) cin += curvature_coeff(dx, lambda[b], kappa[b]);
         kin[b] = make_spec(cin, 1.0, 0.0);
         // per-axis share of dx^2/(i lambda z): dx/sqrt(lambda |z|) * exp(-+ i pi/4)
-        const double a1 = (double)((long double)dx / sqrtl((long double)lambda[b] * fabsl((long double)z)));
-        kout[b] = make_spec(qpf_coeff(dx_out[b], lambda[b], z), a1, (z > 0 ? -0.125 : 0.125) + centred_phase0(p->N, z > 0 ? +1 : -1));
+        const double a1 = (double)((long double)dx / sqrtl((long double)lambda[b] * fabsl(z)));
+        const long double cout = kind != FT_WTS ? qpf_coeff(dx_out[b], lambda[b], z) : 0.0L;
+        kout[b] = make_spec(cout, a1, (fwd ? -0.125 : 0.125) + centred_phase0(p->N, fwd ? +1 : -1));
     }
     // the (-1)^n (odd N: the phase ramp) of the centred transform rides on both tables
     TableRequest r[3];
     int nreq = 2;
-    const int alt = z > 0 ? +1 : -1;
+    const int alt = fwd ? +1 : -1;
     r[0] = request_table(p, KIND_CENTRED, alt, kin, cap);
     r[1] = request_table(p, KIND_CENTRED, alt, kout, cap);
     if (opd) r[nreq++] = request_inv_lambda(p, lambda, cap);
     fresnel_status st = flush_builds(p, r, nreq);
     if (st != FRESNEL_OK) return st;
     const double *il = opd ? (const double *)p->slots[r[2].slot].dev : nullptr;
-    const int mode = z > 0 ? MODE_FWD : MODE_INV;
-    st = run_two_passes(p, mode, wf, p->slots[r[0].slot].dev, p->slots[r[1].slot].dev, amp, opd, il, 1.0, surface);
+    st = run_two_passes(p, fwd ? MODE_FWD : MODE_INV, wf, p->slots[r[0].slot].dev, p->slots[r[1].slot].dev, amp, opd, il, 1.0, surface);
     if (st != FRESNEL_OK) return st;
     for (int b = 0; b < p->batch; ++b) pixel_inout[b] = dx_out[b];
     return FRESNEL_OK;
+}
+
+// [thin lens f] -> [optic phasor] -> direct Fresnel propagation by z
+fresnel_status direct_impl(fresnel_plan *p, void *wf, double *pixel_inout, const double *lambda, double z,
+                           double f, const void *amp, const void *opd, int surface = -1)
+{
+    std::vector<double> zb(p->batch, z);
+    std::vector<long double> kappa;
+    if (std::isfinite(f)) kappa.assign(p->batch, -1.0L / (long double)f);
+    return ft_leg(p, wf, pixel_inout, lambda, zb.data(), FT_DIRECT, kappa.empty() ? nullptr : kappa.data(), amp, opd, surface);
 }
 
 // ---- a run of consecutive angular-spectrum surfaces, fused at train level ---------------------------------------
@@ -1121,6 +1160,126 @@ fresnel_status fresnel_system_run(fresnel_plan *p, void *wf, double *pixel_inout
         if (st != FRESNEL_OK) return finish(st);
         if (method_used) method_used[s] = method[s];
         ++s;
+    }
+    return finish(FRESNEL_OK);
+}
+
+// ---- train of surfaces under the Gaussian pilot-beam rule ------------------------------------------------------
+// Host-side bookkeeping per batch element in long double (the same expressions, in the same order, as the oracle's
+// description of the rule in DESIGN.md reading g21); the array work is the existing two-pass kernels with other
+// tables: PTP = angular-spectrum leg, WTS / STW = single-transform legs without the output / input chirp.
+fresnel_status fresnel_system_run_pilot(fresnel_plan *p, void *wf, double *pixel_inout, const double *lambda,
+                                        const fresnel_surface *surf, int nsurf, double rayleigh_factor,
+                                        fresnel_pilot_state *state, int *legs_used)
+{
+    if (!p || !wf || !state || nsurf < 0 || (nsurf > 0 && !surf) || !(rayleigh_factor > 0)) return FRESNEL_ERR_INVALID_ARG;
+    if (!valid_positive(pixel_inout, p->batch) || !valid_positive(lambda, p->batch)) return FRESNEL_ERR_INVALID_ARG;
+    const int nb = p->batch;
+    for (int b = 0; b < nb; ++b)
+        if (!(state[b].w0 > 0) || !std::isfinite(state[b].zw) || !std::isfinite(state[b].z) || std::isnan(state[b].rref) || state[b].rref == 0.0)
+            return FRESNEL_ERR_INVALID_ARG;
+    for (int s = 0; s < nsurf; ++s)
+        if (std::isnan(surf[s].f) || surf[s].f == 0.0 || !std::isfinite(surf[s].z)) return FRESNEL_ERR_INVALID_ARG;
+    DeviceGuard g(p);
+    const long double rf = rayleigh_factor;
+
+    // ---- dry run: the legs of every surface, for every batch element; nothing is enqueued before the whole train is known
+    struct Step { int leg[2]; bool chirp; std::vector<long double> kappa; std::vector<double> d1, d2; };
+    std::vector<Step> steps(nsurf);
+    std::vector<long double> w0(nb), zw(nb), zc(nb), inv_rref(nb);
+    for (int b = 0; b < nb; ++b) {
+        w0[b] = state[b].w0; zw[b] = state[b].zw; zc[b] = state[b].z;
+        inv_rref[b] = std::isfinite(state[b].rref) ? 1.0L / (long double)state[b].rref : 0.0L;
+    }
+    for (int s = 0; s < nsurf; ++s) {
+        Step &st = steps[s];
+        st.leg[0] = st.leg[1] = 0;
+        st.chirp = false;
+        st.kappa.assign(nb, 0.0L); st.d1.assign(nb, 0.0); st.d2.assign(nb, 0.0);
+        const fresnel_surface &q = surf[s];
+        for (int b = 0; b < nb; ++b) {
+            const long double lam = lambda[b];
+            if (std::isfinite(q.f)) {            // thin lens: ABCD on the pilot beam, residual chirp on the array
+                const long double zR = PI_L * w0[b] * w0[b] / lam;
+                const long double qr = zc[b] - zw[b], qi = zR;
+                const long double den = qr * qr + qi * qi;
+                const long double ir = qr / den - 1.0L / (long double)q.f, ii = -qi / den;
+                const long double d2 = ir * ir + ii * ii;
+                const long double q2r = ir / d2, q2i = -ii / d2;
+                const long double zw2 = zc[b] - q2r, zR2 = q2i;
+                const long double inv_rref2 = (fabsl(zc[b] - zw2) < rf * zR2) ? 0.0L : 1.0L / (zc[b] - zw2);
+                st.kappa[b] = inv_rref[b] - 1.0L / (long double)q.f - inv_rref2;
+                if (st.kappa[b] != 0.0L) st.chirp = true;
+                zw[b] = zw2;
+                w0[b] = sqrtl(lam * zR2 / PI_L);
+                inv_rref[b] = inv_rref2;
+            }
+            int leg[2] = {0, 0};
+            if (q.z != 0.0) {
+                const long double zR = PI_L * w0[b] * w0[b] / lam;
+                const long double z1 = zc[b], z2 = zc[b] + (long double)q.z;
+                const int in1 = inv_rref[b] == 0.0L;
+                const int in2 = fabsl(z2 - zw[b]) < rf * zR;
+                if (in1 && in2) {
+                    leg[0] = 1; st.d1[b] = q.z;
+                } else {
+                    st.d1[b] = (double)(zw[b] - z1); st.d2[b] = (double)(z2 - zw[b]);
+                    if (st.d1[b] != 0.0) leg[0] = in1 ? 1 : 3;
+                    if (st.d2[b] != 0.0) leg[1] = in2 ? 1 : 2;
+                }
+                zc[b] = z2;
+                inv_rref[b] = in2 ? 0.0L : 1.0L / (z2 - zw[b]);
+            }
+            if (b == 0) { st.leg[0] = leg[0]; st.leg[1] = leg[1]; }
+            else if (leg[0] != st.leg[0] || leg[1] != st.leg[1]) return FRESNEL_ERR_UNSUPPORTED;   // the batch straddles a regime boundary
+        }
+        // a single-transform leg needs one sign of dz over the batch
+        for (int l = 0; l < 2; ++l)
+            if (st.leg[l] >= 2) {
+                const std::vector<double> &d = l == 0 ? st.d1 : st.d2;
+                for (int b = 1; b < nb; ++b)
+                    if ((d[b] > 0) != (d[0] > 0)) return FRESNEL_ERR_UNSUPPORTED;
+            }
+    }
+
+    // ---- enqueue ----
+    p->schedule.clear();
+    auto finish = [&](fresnel_status st) {
+        if (st == FRESNEL_OK) train_event(p, p->schedule.size());
+        p->train_ev.clear();
+        return st;
+    };
+    for (int s = 0; s < nsurf; ++s) {
+        const Step &st = steps[s];
+        const fresnel_surface &q = surf[s];
+        const void *amp = q.amp, *opd = q.opd;
+        bool optic_pending = st.chirp || amp || opd;
+        std::vector<ChirpSpec> ck;
+        if (st.chirp) {
+            ck.resize(nb);
+            for (int b = 0; b < nb; ++b) ck[b] = make_spec(curvature_coeff(pixel_inout[b], lambda[b], st.kappa[b]), 1.0, 0.0);
+        }
+        fresnel_status rc = FRESNEL_OK;
+        for (int l = 0; l < 2 && rc == FRESNEL_OK; ++l) {
+            const int leg = st.leg[l];
+            if (leg == 0) continue;
+            const std::vector<double> &d = l == 0 ? st.d1 : st.d2;
+            if (leg == 1) rc = as_leg(p, wf, pixel_inout, lambda, optic_pending ? ck : std::vector<ChirpSpec>(), optic_pending ? amp : nullptr,
+                                      optic_pending ? opd : nullptr, d.data(), s);
+            else rc = ft_leg(p, wf, pixel_inout, lambda, d.data(), leg == 2 ? FT_WTS : FT_STW, (optic_pending && st.chirp) ? st.kappa.data() : nullptr,
+                             optic_pending ? amp : nullptr, optic_pending ? opd : nullptr, s);
+            optic_pending = false;
+        }
+        if (rc == FRESNEL_OK && optic_pending) {         // no propagation leg took the optic along: apply it on its own
+            std::vector<double> zero(nb, 0.0);
+            rc = as_leg(p, wf, pixel_inout, lambda, ck, amp, opd, zero.data(), s);
+        }
+        if (rc != FRESNEL_OK) return finish(rc);
+        if (legs_used) { legs_used[2 * s] = st.leg[0]; legs_used[2 * s + 1] = st.leg[1]; }
+    }
+    for (int b = 0; b < nb; ++b) {
+        state[b].w0 = (double)w0[b]; state[b].zw = (double)zw[b]; state[b].z = (double)zc[b];
+        state[b].rref = inv_rref[b] == 0.0L ? INFINITY : (double)(1.0L / inv_rref[b]);
     }
     return finish(FRESNEL_OK);
 }

@@ -142,13 +142,15 @@ FR_DEV void gen_stage(const typename cplx_of<T>::type *src, typename cplx_of<T>:
 #pragma unroll
         for (int t = 0; t < R; ++t) v[t] = src[(size_t)(b + t * nb) * W + g];
         if (Ns > 1) {
-            int e = 0;                             // (t * k * tstep) mod len, advanced by k*tstep per t
-            const int step = k * tstep;            // < len
+            // W_{Ns R}^{t k} = w^t with w = W_len^{k tstep}: ONE table load, the powers by a product tree (w^t = w^(t/2) *
+            // w^(t - t/2): at most four chained multiplies for t <= 15, so a power is good to a few ulp)
+            C pw[R];
+            pw[1] = ldg_c(tw + k * tstep);         // k * tstep < len
+            v[1] = cmul(v[1], pw[1]);
 #pragma unroll
-            for (int t = 1; t < R; ++t) {
-                e += step;
-                if (e >= len) e -= len;
-                v[t] = cmul(v[t], ldg_c(tw + e));
+            for (int t = 2; t < R; ++t) {
+                pw[t] = (t & 1) ? cmul(pw[t / 2], pw[t - t / 2]) : csq(pw[t / 2]);
+                v[t] = cmul(v[t], pw[t]);
             }
         }
         if constexpr (R == 16) dft16<-1>(v);
@@ -232,7 +234,7 @@ FR_DEV void gen_dft(typename cplx_of<T>::type *&src, typename cplx_of<T>::type *
 }
 
 template <typename T>
-__global__ void __launch_bounds__(kGenThreads) gen_pass_kernel(GenArgs<T> a, const __grid_constant__ CUtensorMap tmap)
+__global__ void __launch_bounds__(kGenThreads, 2) gen_pass_kernel(GenArgs<T> a, const __grid_constant__ CUtensorMap tmap)
 {
     using C = typename cplx_of<T>::type;
     constexpr int ES = (int)sizeof(C);

@@ -70,8 +70,8 @@ enum { FRESNEL_FORWARD = +1, FRESNEL_INVERSE = -1 };
  *   - any other N in [16, 8192] ("N = 2800 ran faster than 4096"; npix = 1025, :259): the
  *     shared-memory path of gen_kernel.cuh -- mixed radix when N = 2^a 3^b 5^c 7^d 11^e 13^f, otherwise Bluestein
  *     (chirp x circular convolution of the next 7-smooth length >= 2N-1 x chirp), as long as two line buffers of the
- *     transform length fit one SM's shared memory (complex128: mixed radix N <= 7200, Bluestein N <= 3600;
- *     complex64: 7200 / 3600 with 16-byte column tiles); beyond that FRESNEL_ERR_UNSUPPORTED.  Odd N: the grid
+ *     transform length fit one SM's shared memory (mixed radix N <= 6700, Bluestein N <= 3350 for both precisions;
+ *     complex64 then takes 16-byte column tiles); beyond that FRESNEL_ERR_UNSUPPORTED.  Odd N: the grid
  *     centre is pixel N/2 (integer division), frequencies in FFT order are q/(N dx) for q <= (N-1)/2 and
  *     (q-N)/(N dx) above, and centred transforms carry phase ramps instead of (-1)^n signs.  Train-level fusion
  *     (fresnel_system_run) applies to power-of-two grids only. */

@@ -27,7 +27,8 @@ constexpr int kGenThreads = 256;
 constexpr int kGenMaxSmem = 226 * 1024;   // dynamic shared memory the generic pass may ask for (227 KB minus its static part)
 
 // bytes of one line buffer (M x W complex), rounded up to the 128-byte alignment TMA wants of a shared-memory box
-__host__ __device__ constexpr size_t gen_buffer_bytes(int M, int W, int es) { return ((size_t)M * W * es + 127) / 128 * 128; }
+// (with room for the padded layout of the intermediate stages: one spare element every 16, see gen_stage)
+__host__ __device__ constexpr size_t gen_buffer_bytes(int M, int W, int es) { return ((size_t)(M + M / 16 + 1) * W * es + 127) / 128 * 128; }
 
 template <typename T> struct GenArgs {
     using C = typename cplx_of<T>::type;
@@ -127,9 +128,14 @@ template <int P, typename C> FR_DEV void dft_odd(C (&v)[P])
     for (int q = 0; q < P; ++q) v[q] = res[q];
 }
 
-// one Stockham stage of radix R over W interleaved lines of length `len`: src -> dst, layout element (n, g) at [n*W + g]
-template <typename T, int R>
-FR_DEV void gen_stage(const typename cplx_of<T>::type *src, typename cplx_of<T>::type *dst, int len, int W, int Ns,
+// one Stockham stage of radix R over W interleaved lines of length `len`: src -> dst, layout element (n, g) at [n*W + g].
+// PIN / POUT: the input / output buffer uses the padded layout n -> n + n/16 (the stride-R scatter of the first stage
+// would otherwise hit the same banks 8 times over); the first stage of a transform reads, and the last one writes, the
+// dense layout that TMA and the pointwise steps use.
+template <bool PADDED> FR_DEV int gen_pos(int n) { return PADDED ? n + (n >> 4) : n; }
+
+template <typename T, int R, bool PIN, bool POUT>
+FR_DEV void gen_stage(const typename cplx_of<T>::type *__restrict__ src, typename cplx_of<T>::type *__restrict__ dst, int len, int W, int Ns,
                       const typename cplx_of<T>::type *__restrict__ tw, int tid)
 {
     using C = typename cplx_of<T>::type;
@@ -140,7 +146,7 @@ FR_DEV void gen_stage(const typename cplx_of<T>::type *src, typename cplx_of<T>:
         const int k = b % Ns;
         C v[R];
 #pragma unroll
-        for (int t = 0; t < R; ++t) v[t] = src[(size_t)(b + t * nb) * W + g];
+        for (int t = 0; t < R; ++t) v[t] = src[(size_t)gen_pos<PIN>(b + t * nb) * W + g];
         if (Ns > 1) {
             // W_{Ns R}^{t k} = w^t with w = W_len^{k tstep}: ONE table load, the powers by a product tree (w^t = w^(t/2) *
             // w^(t - t/2): at most four chained multiplies for t <= 15, so a power is good to a few ulp)
@@ -160,8 +166,16 @@ FR_DEV void gen_stage(const typename cplx_of<T>::type *src, typename cplx_of<T>:
         else dft_odd<R>(v);
         const int o = (b - k) * R + k;
 #pragma unroll
-        for (int q = 0; q < R; ++q) dst[(size_t)(o + q * Ns) * W + g] = v[q];
+        for (int q = 0; q < R; ++q) dst[(size_t)gen_pos<POUT>(o + q * Ns) * W + g] = v[q];
     }
+}
+
+template <typename T, int R>
+FR_DEV void gen_stage_any(const typename cplx_of<T>::type *src, typename cplx_of<T>::type *dst, int len, int W, int Ns,
+                          const typename cplx_of<T>::type *__restrict__ tw, int tid, bool pin, bool pout)
+{
+    if (pin) { if (pout) gen_stage<T, R, true, true>(src, dst, len, W, Ns, tw, tid); else gen_stage<T, R, true, false>(src, dst, len, W, Ns, tw, tid); }
+    else     { if (pout) gen_stage<T, R, false, true>(src, dst, len, W, Ns, tw, tid); else gen_stage<T, R, false, false>(src, dst, len, W, Ns, tw, tid); }
 }
 
 // forward transform of length len = a.M on the W lines in *src; on return *src holds the result (buffers swapped as needed)
@@ -172,16 +186,17 @@ FR_DEV void gen_fft(typename cplx_of<T>::type *&src, typename cplx_of<T>::type *
     int Ns = 1;
     for (int s = 0; s < a.nstages; ++s) {
         const int R = a.radix[s];
+        const bool pin = s > 0, pout = s + 1 < a.nstages;
         switch (R) {
-        case 16: gen_stage<T, 16>(src, dst, a.M, a.W, Ns, a.tw, tid); break;
-        case 8:  gen_stage<T, 8>(src, dst, a.M, a.W, Ns, a.tw, tid); break;
-        case 4:  gen_stage<T, 4>(src, dst, a.M, a.W, Ns, a.tw, tid); break;
-        case 2:  gen_stage<T, 2>(src, dst, a.M, a.W, Ns, a.tw, tid); break;
-        case 3:  gen_stage<T, 3>(src, dst, a.M, a.W, Ns, a.tw, tid); break;
-        case 5:  gen_stage<T, 5>(src, dst, a.M, a.W, Ns, a.tw, tid); break;
-        case 7:  gen_stage<T, 7>(src, dst, a.M, a.W, Ns, a.tw, tid); break;
-        case 11: gen_stage<T, 11>(src, dst, a.M, a.W, Ns, a.tw, tid); break;
-        default: gen_stage<T, 13>(src, dst, a.M, a.W, Ns, a.tw, tid); break;
+        case 16: gen_stage_any<T, 16>(src, dst, a.M, a.W, Ns, a.tw, tid, pin, pout); break;
+        case 8:  gen_stage_any<T, 8>(src, dst, a.M, a.W, Ns, a.tw, tid, pin, pout); break;
+        case 4:  gen_stage_any<T, 4>(src, dst, a.M, a.W, Ns, a.tw, tid, pin, pout); break;
+        case 2:  gen_stage_any<T, 2>(src, dst, a.M, a.W, Ns, a.tw, tid, pin, pout); break;
+        case 3:  gen_stage_any<T, 3>(src, dst, a.M, a.W, Ns, a.tw, tid, pin, pout); break;
+        case 5:  gen_stage_any<T, 5>(src, dst, a.M, a.W, Ns, a.tw, tid, pin, pout); break;
+        case 7:  gen_stage_any<T, 7>(src, dst, a.M, a.W, Ns, a.tw, tid, pin, pout); break;
+        case 11: gen_stage_any<T, 11>(src, dst, a.M, a.W, Ns, a.tw, tid, pin, pout); break;
+        default: gen_stage_any<T, 13>(src, dst, a.M, a.W, Ns, a.tw, tid, pin, pout); break;
         }
         Ns *= R;
         __syncthreads();
@@ -190,19 +205,15 @@ FR_DEV void gen_fft(typename cplx_of<T>::type *&src, typename cplx_of<T>::type *
 }
 
 // length-N forward DFT of the W lines in *src (first N entries of each line valid; the rest is scratch).
-//   conj_in:  the input is conjugated on the way in (first half of an inverse transform);
-//   post:     optional [N] table multiplied in afterwards (per batch element), conj_out: result conjugated first.
+//   conj_in (Bluestein only): the input is conjugated on the way in (first half of an inverse transform) -- folded into
+//   the chirp multiply; in the mixed-radix case the CALLER conjugates inside its neighbouring pointwise step.
 // Mixed radix: the transform itself.  Bluestein: chirp, zero-pad, FFT_M, x filter, inverse FFT_M, chirp.
 template <typename T>
 FR_DEV void gen_dft(typename cplx_of<T>::type *&src, typename cplx_of<T>::type *&dst, const GenArgs<T> &a, int tid, bool conj_in)
 {
     using C = typename cplx_of<T>::type;
     const int N = a.N, M = a.M, W = a.W;
-    if (a.blu_w == nullptr) {
-        if (conj_in) {
-            for (int e = tid; e < N * W; e += kGenThreads) src[e].y = -src[e].y;
-            __syncthreads();
-        }
+    if (a.blu_w == nullptr) {            // mixed radix: the caller has folded the conjugation into its own pointwise step
         gen_fft<T>(src, dst, a, tid);
         return;
     }
@@ -289,34 +300,38 @@ __global__ void __launch_bounds__(kGenThreads, 2) gen_pass_kernel(GenArgs<T> a, 
         }
     }
     // pre table (along the line) and, for MODE_INV, the conjugation that opens an inverse transform
-    const bool inv = a.mode == MODE_INV;
-    if (a.pre != nullptr) {
-        const C *p = a.pre + (size_t)b * N;
-        for (int e = tid; e < N * W; e += kGenThreads) src[e] = cmul(src[e], ldg_c(p + e / W));
+    const bool inv = a.mode == MODE_INV, conv = a.mode == MODE_CONV, blu = a.blu_w != nullptr;
+    if (a.pre != nullptr || (inv && !blu)) {
+        const C *p = a.pre != nullptr ? a.pre + (size_t)b * N : nullptr;
+        for (int e = tid; e < N * W; e += kGenThreads) {
+            C x = src[e];
+            if (p != nullptr) x = cmul(x, ldg_c(p + e / W));
+            if (inv && !blu) x.y = -x.y;
+            src[e] = x;
+        }
     }
     __syncthreads();
 
-    gen_dft<T>(src, dst, a, tid, inv);                       // F (or conj . F . with the closing conj below)
+    gen_dft<T>(src, dst, a, tid, inv && blu);                // F (or conj . F . with the closing conj below)
     {
         const C *m = a.mid != nullptr ? a.mid + (size_t)b * N : nullptr;
-        const bool conv = a.mode == MODE_CONV;
-        for (int e = tid; e < N * W; e += kGenThreads) {
-            C x = src[e];
-            if (inv) x.y = -x.y;                             // closes the inverse transform
-            if (m != nullptr) x = cmul(x, ldg_c(m + e / W));
-            src[e] = x;
-        }
-        __syncthreads();
-        if (conv) {
-            gen_dft<T>(src, dst, a, tid, true);              // inverse transform = conj . F . conj
-            for (int e = tid; e < N * W; e += kGenThreads) src[e].y = -src[e].y;
+        if (inv || m != nullptr || (conv && !blu)) {
+            for (int e = tid; e < N * W; e += kGenThreads) {
+                C x = src[e];
+                if (inv) x.y = -x.y;                         // closes the inverse transform
+                if (m != nullptr) x = cmul(x, ldg_c(m + e / W));
+                if (conv && !blu) x.y = -x.y;                // opens the inverse transform of the convolution
+                src[e] = x;
+            }
             __syncthreads();
         }
+        if (conv) gen_dft<T>(src, dst, a, tid, blu);         // inverse transform = conj . F . conj (closing conj: on the store)
     }
     // ---- scale, per-row factor, store ----
+    const T sx = a.scale, sy = conv ? -a.scale : a.scale;   // scale, and the closing conjugation of the convolution
     if (a.col == 1) {
-        if (a.scale != (T)1)
-            for (int e = tid; e < N * W; e += kGenThreads) { src[e].x *= a.scale; src[e].y *= a.scale; }
+        if (a.scale != (T)1 || conv)
+            for (int e = tid; e < N * W; e += kGenThreads) { src[e].x *= sx; src[e].y *= sy; }
         fence_async_proxy();
         __syncthreads();
         if (tid == 0) {
@@ -327,7 +342,7 @@ __global__ void __launch_bounds__(kGenThreads, 2) gen_pass_kernel(GenArgs<T> a, 
         C *g0 = a.wf + (size_t)b * N * N + line0;
         for (int e = tid; e < N * W; e += kGenThreads) {
             const int n = e / W, g = e - n * W;
-            if (g < nl) { C x = src[e]; x.x *= a.scale; x.y *= a.scale; g0[(size_t)n * N + g] = x; }
+            if (g < nl) { C x = src[e]; x.x *= sx; x.y *= sy; g0[(size_t)n * N + g] = x; }
         }
     } else {
         for (int g = 0; g < nl; ++g) {
@@ -338,7 +353,11 @@ __global__ void __launch_bounds__(kGenThreads, 2) gen_pass_kernel(GenArgs<T> a, 
                 const C c = ldg_c(a.rowfac + (size_t)b * N + line0 + g);
                 rf.x = c.x * a.scale; rf.y = c.y * a.scale;
             }
-            for (int n = tid; n < N; n += kGenThreads) row[n] = cmul(src[(size_t)n * W + g], rf);
+            for (int n = tid; n < N; n += kGenThreads) {
+                C x = src[(size_t)n * W + g];
+                if (conv) x.y = -x.y;
+                row[n] = cmul(x, rf);
+            }
         }
     }
 }

@@ -54,3 +54,29 @@ def whole_job_rate(units_this_rank: float, seconds_this_rank: float, device=None
     total = sum_over_ranks([units_this_rank], device)[0]
     slowest = max_over_ranks([seconds_this_rank], device)[0]
     return total / slowest
+
+
+def sharded_polychromatic_image(make_plan, wavefront_of, dx, lam, weights, run_train, new_image, rank: int, world: int):
+    """The multi-GPU data path of a broadband image (PAPER.md:51 "repeated for all of the wavelengths", :63 one process
+    per wavelength; SURVEY.md sec. 8(e)): the `len(lam)` wavelengths are split into contiguous slices, one per rank;
+    every rank propagates ITS wavelengths through the train, accumulates sum_b w_b |U_b|^2 over them
+    (fresnel_accumulate_intensity) and ONE sum all-reduce of the N x N image finishes the job on every rank.  No
+    communication happens during propagation.
+
+    The caller supplies the pieces that touch the device, so the same code runs on GPUs (bench.py, NCCL) and in the
+    CPU test with the library stubbed out at the Plan boundary (gloo):
+        make_plan(batch_local)            -> plan with .accumulate_intensity(wf, weights, image)
+        wavefront_of(lo, hi)              -> this rank's wavefronts [hi-lo][N][N] (device tensor)
+        run_train(plan, wf, dx_l, lam_l)  -> propagate in place (e.g. plan.system_run)
+        new_image()                       -> zeroed real [N][N] tensor on the device
+    Returns (image, (lo, hi), plan, wf)."""
+    lo, hi = shard_batch(len(lam), rank, world)
+    if hi == lo:
+        raise ValueError(f"rank {rank}: no wavelength left ({len(lam)} wavelengths over {world} ranks)")
+    plan = make_plan(hi - lo)
+    wf = wavefront_of(lo, hi)
+    run_train(plan, wf, dx[lo:hi], lam[lo:hi])
+    image = new_image()
+    plan.accumulate_intensity(wf, weights[lo:hi], image)
+    reduce_image(image)
+    return image, (lo, hi), plan, wf

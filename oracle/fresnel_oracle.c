@@ -28,7 +28,7 @@
  * ran N = 2800; App. B gives npix = 1025, :259) through the plain separable
  * O(N^3) DFT of item 2b -- no FFT cleverness for those.
  *
- * Parity pins: every function here is pinned in tests/test_oracle_pins.py (P0..P23 of
+ * Parity pins: every function here is pinned in tests/test_oracle_pins.py (P0..P26 of
  * DESIGN.md) against closed forms / exact identities / brute force.  Nothing is
  * "parity unpinned".
  */
@@ -632,5 +632,69 @@ int oracle_system_run_pilot(double *u, int N, double *dx_inout, double lambda, i
     }
     state[0] = (double)w0; state[1] = (double)zw; state[2] = (double)zc;
     state[3] = inv_rref == 0.0L ? INFINITY : (double)(1.0L / inv_rref);
+    return ORACLE_OK;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * Fraunhofer propagation by a matrix Fourier transform ("discrete matrix
+ * Fourier transforms of modest sized arrays", :119; reading g22).
+ *
+ * The field in the focal plane of a lens of focal length f, sampled on ANY output grid (nb x nb pixels of pitch
+ * dx_out, origin on pixel nb/2), from an na x na input of pitch dx_in (origin on pixel na/2):
+ *     V[p,q] = s * sum_j sum_k  U[j,k] * exp(-+ 2 pi i (x_k x'_q + y_j y'_p) / (lambda f)),    s = dx_in^2 / (+- i lambda f)
+ * upper signs for direction = +1 (forward kernel), lower for -1 (the inverse pair: with dx_out = lambda f/(na dx_in)
+ * and nb = na, inverse o forward = identity).  It is the Fourier core of the direct Fresnel transform (item 6) freed
+ * from the FFT's sampling: at dx_out = lambda f/(na dx_in), nb = na, it equals s * fftshift(fft2(ifftshift(U))).
+ * Written out as the definition: the two kernel matrices E_x[q,k], E_y[p,j] from per-entry long-double phases,
+ * then the two plain matrix products  T = U E_x^T,  V = s E_y T  accumulated in double (O(na^2 nb + na nb^2)).
+ * u: na x na interleaved complex, v: nb x nb interleaved complex (written), both host.
+ * ------------------------------------------------------------------------------------------ */
+int oracle_mft(const double *u, int na, double dx_in, double *v, int nb, double dx_out, double lambda, double f, int direction)
+{
+    if (!u || !v || na <= 0 || nb <= 0 || !(dx_in > 0) || !(dx_out > 0) || !(lambda > 0) || !isfinite(f) || f == 0.0) return ORACLE_ERR_INVALID_ARG;
+    if (direction != 1 && direction != -1) return ORACLE_ERR_INVALID_ARG;
+    double *e = (double *)malloc(2 * (size_t)nb * na * sizeof(double));      /* E[q,k] = exp(-+ 2 pi i x_k x'_q/(lambda f)) (same for x and y) */
+    double *t = (double *)malloc(2 * (size_t)na * nb * sizeof(double));      /* T[j,q] */
+    if (!e || !t) { free(e); free(t); return ORACLE_ERR_ALLOC; }
+    const long double sgn = direction > 0 ? -1.0L : 1.0L;
+#pragma omp parallel for num_threads(nthreads()) schedule(static)
+    for (int q = 0; q < nb; ++q) {
+        const long double xq = (long double)(q - nb / 2) * (long double)dx_out;
+        for (int k = 0; k < na; ++k) {
+            const long double xk = (long double)(k - na / 2) * (long double)dx_in;
+            const long double th = sgn * 2.0L * PI_L * xk * xq / ((long double)lambda * (long double)f);
+            e[2 * ((size_t)q * na + k)] = (double)cosl(th);
+            e[2 * ((size_t)q * na + k) + 1] = (double)sinl(th);
+        }
+    }
+#pragma omp parallel for num_threads(nthreads()) schedule(static)
+    for (int j = 0; j < na; ++j)                                             /* T[j,q] = sum_k U[j,k] E[q,k] */
+        for (int q = 0; q < nb; ++q) {
+            double sr = 0.0, si = 0.0;
+            for (int k = 0; k < na; ++k) {
+                const double ar = u[2 * ((size_t)j * na + k)], ai = u[2 * ((size_t)j * na + k) + 1];
+                const double br = e[2 * ((size_t)q * na + k)], bi = e[2 * ((size_t)q * na + k) + 1];
+                sr += ar * br - ai * bi;
+                si += ar * bi + ai * br;
+            }
+            t[2 * ((size_t)j * nb + q)] = sr;
+            t[2 * ((size_t)j * nb + q) + 1] = si;
+        }
+    /* s = dx^2/(+- i lambda f) = -+ i g,  g = dx^2/(lambda f) */
+    const double g = (double)((long double)dx_in * (long double)dx_in / ((long double)lambda * (long double)f));
+#pragma omp parallel for num_threads(nthreads()) schedule(static)
+    for (int p = 0; p < nb; ++p)                                             /* V[p,q] = s sum_j E[p,j] T[j,q] */
+        for (int q = 0; q < nb; ++q) {
+            double sr = 0.0, si = 0.0;
+            for (int j = 0; j < na; ++j) {
+                const double ar = e[2 * ((size_t)p * na + j)], ai = e[2 * ((size_t)p * na + j) + 1];
+                const double br = t[2 * ((size_t)j * nb + q)], bi = t[2 * ((size_t)j * nb + q) + 1];
+                sr += ar * br - ai * bi;
+                si += ar * bi + ai * br;
+            }
+            if (direction > 0) { v[2 * ((size_t)p * nb + q)] = si * g;  v[2 * ((size_t)p * nb + q) + 1] = -sr * g; }   /* x (-i g) */
+            else               { v[2 * ((size_t)p * nb + q)] = -si * g; v[2 * ((size_t)p * nb + q) + 1] = sr * g; }    /* x (+i g) */
+        }
+    free(e); free(t);
     return ORACLE_OK;
 }

@@ -55,6 +55,8 @@ def lib():
         L.oracle_system_run_pilot.argtypes = [dp, ctypes.c_int, dp, ctypes.c_double, ctypes.c_int, dp, pp, pp, dp,
                                               ctypes.c_double, dp, ctypes.POINTER(ctypes.c_int)]
         L.oracle_system_run_pilot.restype = ctypes.c_int
+        L.oracle_mft.argtypes = [dp, ctypes.c_int, ctypes.c_double, dp, ctypes.c_int, ctypes.c_double, ctypes.c_double, ctypes.c_double, ctypes.c_int]
+        L.oracle_mft.restype = ctypes.c_int
         L.oracle_accumulate_intensity.argtypes = [dp, ctypes.c_int, ctypes.c_double, dp]
         L.oracle_accumulate_intensity.restype = ctypes.c_int
         for name in ("oracle_dft2_naive", "oracle_fft2", "oracle_fftshift", "oracle_ifftshift", "oracle_fft2d",
@@ -279,3 +281,11 @@ def system_run_pilot(u, dx, lam, surfaces, w0, rayleigh_factor=1.0, state=None):
                                          z.ctypes.data_as(dp), float(rayleigh_factor), st.ctypes.data_as(dp),
                                          legs.ctypes.data_as(ctypes.POINTER(ctypes.c_int))), "system_run_pilot")
     return a, dxv.value, tuple(float(x) for x in st[:4]), [(int(legs[2 * i]), int(legs[2 * i + 1])) for i in range(n)]
+
+
+def mft(u, dx_in, nb, dx_out, lam, f, direction=+1):
+    """Fraunhofer propagation by a matrix Fourier transform onto an nb x nb grid of pitch dx_out (NEXT-4)."""
+    a, na = _prep(u)
+    out = np.zeros((int(nb), int(nb)), dtype=np.complex128)
+    _check(lib().oracle_mft(_dptr(a), na, float(dx_in), _dptr(out), int(nb), float(dx_out), float(lam), float(f), int(direction)), "mft")
+    return out

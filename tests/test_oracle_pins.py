@@ -671,3 +671,82 @@ def test_P23_pilot_masks_rayleigh_factor_and_errors(oracle):
         oracle.system_run_pilot(u, dx, lam, [Surface(0.0, 0.1)], w0)
     with pytest.raises(oracle.OracleError):
         oracle.system_run_pilot(u, dx, lam, [Surface(math.inf, 0.1)], -1.0)
+
+
+# ---- P24-P26: Fraunhofer matrix Fourier transform (reading g22) ----
+def test_P24_mft_equals_the_centred_fft_at_critical_sampling(oracle):
+    """At dx_out = lambda f/(na dx_in), nb = na the matrix transform IS the Fourier core of direct Fresnel:
+    dx^2/(i lambda f) fftshift(fft2(ifftshift(U))) -- ties it to the pinned FFT (even, odd and non-power-of-two na);
+    the inverse direction undoes it; and direct Fresnel itself is chirp x MFT x chirp."""
+    lam, f = 0.8e-6, 0.7
+    for na in (64, 45, 100):
+        dx = 1.5e-5
+        u = rnd(na, 240 + na)
+        dxo = lam * f / (na * dx)
+        v = oracle.mft(u, dx, na, dxo, lam, f, +1)
+        want = dx * dx / (1j * lam * f) * np.fft.fftshift(np.fft.fft2(np.fft.ifftshift(u)))
+        assert rel(v, want) <= 1e-12
+        assert rel(v, dx * dx / (1j * lam * f) * oracle.fft2d(u, +1, True)) <= 1e-12
+        assert rel(oracle.mft(v, dxo, na, dx, lam, f, -1), u) <= 1e-12
+    na, dx = 64, 1.5e-5
+    u = rnd(na, 241)
+    z = 0.4
+    d, dxo = oracle.propagate_direct(u, dx, lam, z)
+    m = oracle.mft(oracle.apply_qpf(u, dx, lam, z), dx, na, dxo, lam, z, +1)
+    assert rel(oracle.apply_qpf(m, dxo, lam, z), d) <= 1e-12
+
+
+def test_P25_mft_closed_forms(oracle):
+    """Closed forms on an output grid the FFT cannot reach (nb != na, 3.7x finer than critical): the centre sample is
+    sum(U) dx^2/(i lambda f) exactly; a uniform square aperture gives the product of two Dirichlet kernels; a shifted
+    delta gives a pure phase ramp of the right sign and slope; linearity and separability."""
+    lam, f, na, dx, nb = 1e-6, 0.5, 48, 2e-5, 37
+    dxo = lam * f / (na * dx) / 3.7
+    u = rnd(na, 250)
+    v = oracle.mft(u, dx, nb, dxo, lam, f, +1)
+    assert v[nb // 2, nb // 2] == pytest.approx(u.sum() * dx * dx / (1j * lam * f), rel=1e-12)
+    # square aperture of half-width h pixels (indices -h..h): sum_k exp(-2 pi i k a) = sin(pi (2h+1) a)/sin(pi a), a = dx x'/(lam f)
+    h = 7
+    sq = np.zeros((na, na))
+    sq[na // 2 - h:na // 2 + h + 1, na // 2 - h:na // 2 + h + 1] = 1.0
+    a = dx * (np.arange(nb) - nb // 2) * dxo / (lam * f)
+    with np.errstate(invalid="ignore", divide="ignore"):
+        dk = np.where(a == 0, 2 * h + 1, np.sin(np.pi * (2 * h + 1) * a) / np.sin(np.pi * a))
+    want = dx * dx / (1j * lam * f) * dk[:, None] * dk[None, :]
+    assert rel(oracle.mft(sq, dx, nb, dxo, lam, f, +1), want) <= 1e-12
+    # delta at pixel (j0, k0): exp(-2 pi i (x_k0 x' + y_j0 y')/(lam f)) -- and the conjugate ramp for the inverse kernel
+    j0, k0 = na // 2 + 5, na // 2 - 3
+    d = np.zeros((na, na), complex)
+    d[j0, k0] = 1.0
+    xo = (np.arange(nb) - nb // 2) * dxo
+    ramp = np.exp(-2j * np.pi * ((k0 - na // 2) * dx * xo[None, :] + (j0 - na // 2) * dx * xo[:, None]) / (lam * f))
+    assert rel(oracle.mft(d, dx, nb, dxo, lam, f, +1), dx * dx / (1j * lam * f) * ramp) <= 1e-13
+    assert rel(oracle.mft(d, dx, nb, dxo, lam, f, -1), dx * dx / (-1j * lam * f) * np.conj(ramp)) <= 1e-13
+    w = rnd(na, 251)
+    assert rel(oracle.mft(2.0 * u - 1j * w, dx, nb, dxo, lam, f, +1), 2.0 * v - 1j * oracle.mft(w, dx, nb, dxo, lam, f, +1)) <= 1e-13
+
+
+def test_P26_mft_airy_pattern_oversampled(oracle):
+    """The use the paper names (a coronagraph's focal plane at high sampling over a small field): circular aperture of
+    radius a -> Airy amplitude (pi a^2/(lam f)) 2 J1(v)/v, v = 2 pi a r'/(lam f), sampled 8x finer than the FFT would,
+    over +-3 Airy rings; the pixelated disc matches the continuous pattern to a fraction of a per cent of the peak
+    (as P8), and the first null sits at 0.61 lam f / a."""
+    from paper_1806_06467_b200 import inputs
+    lam, f, na, dx = 1e-6, 0.5, 256, 1e-5
+    a_px = 100
+    ap = inputs.circular_aperture(na, a_px)
+    nb = 96
+    dxo = lam * f / (na * dx) / 8.0
+    v = oracle.mft(ap, dx, nb, dxo, lam, f, +1)
+    c = nb // 2
+    assert v[c, c] == pytest.approx(ap.sum() * dx * dx / (1j * lam * f), rel=1e-12)
+    xo = (np.arange(nb) - c) * dxo
+    r = np.hypot(xo[None, :], xo[:, None])
+    arg = 2 * np.pi * a_px * dx * r / (lam * f)
+    with np.errstate(invalid="ignore", divide="ignore"):
+        airy = np.where(arg == 0, 1.0, 2 * j1(arg) / arg)
+    want = (np.pi * (a_px * dx) ** 2 / (lam * f)) * airy
+    assert np.abs(np.abs(v) - np.abs(want)).max() <= 4e-3 * np.abs(want).max()
+    prof = np.abs(v[c, c:])
+    null_px = next(i for i in range(1, 40) if prof[i] < prof[i - 1] and prof[i] < prof[i + 1])      # first local minimum
+    assert null_px == pytest.approx(0.6098 * lam * f / (a_px * dx) / dxo, abs=1.0)

@@ -234,6 +234,23 @@ fresnel_status fresnel_system_run_pilot(fresnel_plan *p, void *wf, double *pixel
                                         const fresnel_surface *surf, int nsurf, double rayleigh_factor,
                                         fresnel_pilot_state *state, int *legs_used);
 
+/* Fraunhofer propagation by a MATRIX FOURIER TRANSFORM ("discrete matrix Fourier transforms of modest
+ * sized arrays", :119; reading g22): the field in the focal plane of a lens of
+ * focal length f on ANY output grid -- nb x nb pixels of pitch pixel_out[b], centred on pixel nb/2 -- from the plan's
+ * N x N input of pitch pixel_in[b] (centred on pixel N/2):
+ *     out[b][p][q] = s * sum_j sum_k in[b][j][k] * exp(-+ 2 pi i (x_k x'_q + y_j y'_p) / (lambda_b f)),   s = dx^2/(+- i lambda_b f)
+ * (upper signs: FRESNEL_FORWARD; lower: FRESNEL_INVERSE, the inverse pair at critical sampling).  With
+ * pixel_out = lambda f/(N pixel_in) and nb = N it is the Fourier core of fresnel_propagate_direct; with a finer pitch
+ * and a small nb it is the high-resolution, small-field transform coronagraph models use.  The one dense contraction
+ * of the library: two complex GEMMs (cost 8 (N^2 nb + N nb^2) flops) on the FP64 tensor cores (DMMA) -- complex64 plans
+ * convert on load and round on store.  in: device, [batch][N][N] of the plan's dtype, read only; out: device,
+ * [batch][nb][nb] of the plan's dtype, written; must not alias.  Workspace (kernel matrix and intermediate, 32 batch N nb
+ * bytes) is allocated on first use of a larger nb -- call fresnel_plan_reserve_mft first to keep fresnel_mft itself
+ * allocation-free (required before capturing it into a CUDA graph: FRESNEL_ERR_ALLOC otherwise). */
+fresnel_status fresnel_plan_reserve_mft(fresnel_plan *p, int nb_max);
+fresnel_status fresnel_mft(fresnel_plan *p, const void *in, void *out, int nb, const double *pixel_in, const double *pixel_out,
+                           const double *lambda, double f, int direction);
+
 /* Broadband (polychromatic) image: the incoherent, weighted sum of the batch's monochromatic intensities
  * ("calculations must be repeated for all of the wavelengths"; one process per wavelength in
  * the paper):

@@ -29,7 +29,7 @@ SYMBOLS = (
     "fresnel_plan_create", "fresnel_plan_set_stream", "fresnel_plan_synchronize", "fresnel_plan_destroy",
     "fresnel_plan_launch_count", "fresnel_plan_record_pass_events", "fresnel_plan_record_train_events",
     "fresnel_plan_last_schedule", "fresnel_plan_reserve_tables", "fresnel_plan_release_graph_tables", "fresnel_apply_qpf", "fresnel_apply_mask", "fresnel_fft2d",
-    "fresnel_propagate_as", "fresnel_propagate_direct", "fresnel_surface_as", "fresnel_system_run", "fresnel_system_run_pilot", "fresnel_accumulate_intensity", "fresnel_memcpy_h2d",
+    "fresnel_propagate_as", "fresnel_propagate_direct", "fresnel_surface_as", "fresnel_system_run", "fresnel_system_run_pilot", "fresnel_plan_reserve_mft", "fresnel_mft", "fresnel_accumulate_intensity", "fresnel_memcpy_h2d",
     "fresnel_memcpy_d2h", "fresnel_status_string", "fresnel_version",
 )
 
@@ -90,6 +90,8 @@ def lib() -> ctypes.CDLL:
     L.fresnel_surface_as.argtypes = [vp, vp, dp, dp, cd, vp, vp, cd]
     L.fresnel_system_run.argtypes = [vp, vp, dp, dp, ctypes.POINTER(_Surface), ci, ctypes.POINTER(ci)]
     L.fresnel_system_run_pilot.argtypes = [vp, vp, dp, dp, ctypes.POINTER(_Surface), ci, cd, ctypes.POINTER(_PilotState), ctypes.POINTER(ci)]
+    L.fresnel_plan_reserve_mft.argtypes = [vp, ci]
+    L.fresnel_mft.argtypes = [vp, vp, vp, ci, dp, dp, dp, cd, ci]
     L.fresnel_accumulate_intensity.argtypes = [vp, vp, dp, vp]
     L.fresnel_memcpy_h2d.argtypes = [vp, vp, vp, ctypes.c_size_t]
     L.fresnel_memcpy_d2h.argtypes = [vp, vp, vp, ctypes.c_size_t]
@@ -296,6 +298,20 @@ class Plan:
         self._chk(lib().fresnel_system_run_pilot(self._h, self._wf(wf), pp, lp, arr, n, float(rayleigh_factor), st, legs),
                   "fresnel_system_run_pilot")
         return pa, [(st[b].w0, st[b].zw, st[b].z, st[b].rref) for b in range(self.batch)], [(int(legs[2 * i]), int(legs[2 * i + 1])) for i in range(n)]
+
+    def reserve_mft(self, nb_max: int) -> None:
+        self._chk(lib().fresnel_plan_reserve_mft(self._h, int(nb_max)), "fresnel_plan_reserve_mft")
+
+    def mft(self, wf, out, pixel_in, pixel_out, lam, f: float, direction: int = FORWARD) -> None:
+        """Fraunhofer matrix Fourier transform of wf ([batch][N][N]) onto out ([batch][nb][nb], same dtype)."""
+        nb = int(out.shape[-1])
+        if out.dtype != self.cdtype or not out.is_cuda or not out.is_contiguous() or out.numel() != self.batch * nb * nb:
+            raise ValueError("out must be a contiguous CUDA tensor [batch][nb][nb] of the plan's dtype")
+        _, pi = _darr(pixel_in, self.batch)
+        _, po = _darr(pixel_out, self.batch)
+        _, lp = _darr(lam, self.batch)
+        self._chk(lib().fresnel_mft(self._h, self._wf(wf), ctypes.c_void_p(out.data_ptr()), nb, pi, po, lp, float(f), int(direction)),
+                  "fresnel_mft")
 
     def accumulate_intensity(self, wf, weight, image) -> None:
         """image += sum_b weight[b] * |wf[b]|^2 (image: real N x N device tensor of the plan's precision)."""

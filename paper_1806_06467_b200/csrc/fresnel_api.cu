@@ -14,6 +14,7 @@
 #include "../../include/fresnel.h"
 #include "dispatch.h"
 #include "gen_kernel.cuh"
+#include "mft.cuh"
 #include "pointwise.cuh"
 #include "tables.cuh"
 
@@ -86,6 +87,11 @@ struct fresnel_plan {
     int gen_wcol = 1, gen_box_rows = 256;
     bool gen_tma = false;               // column tiles by TMA (needs a 16-byte multiple row pitch: not complex64 with odd N)
     void *gen_tw = nullptr, *gen_blu_w = nullptr, *gen_blu_b = nullptr;
+    // matrix Fourier transform (mft.cuh): kernel matrix E [batch][nb][N], intermediate T^t [batch][nb][N], per-batch scalars
+    double2 *mft_e = nullptr, *mft_t = nullptr;
+    double *mft_scal = nullptr;         // [4][batch]: c_hi, c_lo, alpha.re, alpha.im  (alpha interleaved at +2*batch)
+    int mft_nb_cap = 0;
+    std::vector<double> mft_key;        // what mft_e currently holds (nb, direction, c_hi.., c_lo..); empty: nothing
     CUtensorMap tmap{};                  // tensor map of the wavefront last seen by the column pass
     const void *tmap_wf = nullptr;
     std::vector<MapDesc> map_descs;     // tensor maps of surface maps, by pointer
@@ -956,6 +962,9 @@ fresnel_status fresnel_plan_destroy(fresnel_plan *p)
         cudaFree(p->gen_tw);
         cudaFree(p->gen_blu_w);
         cudaFree(p->gen_blu_b);
+        cudaFree(p->mft_e);
+        cudaFree(p->mft_t);
+        cudaFree(p->mft_scal);
         for (void *a : p->arenas) cudaFree(a);
         if (p->order_ev) cudaEventDestroy(p->order_ev);
         cudaGetLastError();
@@ -1282,6 +1291,119 @@ fresnel_status fresnel_system_run_pilot(fresnel_plan *p, void *wf, double *pixel
         state[b].rref = inv_rref[b] == 0.0L ? INFINITY : (double)(1.0L / inv_rref[b]);
     }
     return finish(FRESNEL_OK);
+}
+
+// ---- Fraunhofer propagation by a matrix Fourier transform ----------------------------------------------------------
+} // extern "C"
+
+namespace {
+
+struct MftScalArgs {
+    double *dst;                // [4][batch]
+    int batch, b0, n;
+    double v[4][32];
+};
+__global__ void mft_scalars_kernel(MftScalArgs a)
+{
+    const int i = threadIdx.x;
+    if (i < a.n)
+        for (int r = 0; r < 4; ++r) a.dst[(size_t)r * a.batch + a.b0 + i] = a.v[r][i];
+}
+__global__ void mft_alpha_kernel(const double *scal, double2 *alpha, int batch)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < batch) alpha[i] = make_double2(scal[(size_t)2 * batch + i], scal[(size_t)3 * batch + i]);
+}
+
+fresnel_status mft_reserve(fresnel_plan *p, int nb)
+{
+    if (nb <= p->mft_nb_cap) return FRESNEL_OK;
+    if (capture_state(p).active) return FRESNEL_ERR_ALLOC;                 // allocates: reserve before capturing
+    cudaStreamSynchronize(p->stream);
+    cudaFree(p->mft_e); cudaFree(p->mft_t);
+    p->mft_e = p->mft_t = nullptr;
+    p->mft_nb_cap = 0;
+    p->mft_key.clear();
+    const size_t n = (size_t)p->batch * nb * p->N;
+    if (cudaMalloc((void **)&p->mft_e, n * sizeof(double2)) != cudaSuccess || cudaMalloc((void **)&p->mft_t, n * sizeof(double2)) != cudaSuccess) {
+        cudaGetLastError();
+        cudaFree(p->mft_e); p->mft_e = nullptr;
+        return FRESNEL_ERR_ALLOC;
+    }
+    if (!p->mft_scal && cudaMalloc((void **)&p->mft_scal, (size_t)6 * p->batch * sizeof(double)) != cudaSuccess) { cudaGetLastError(); return FRESNEL_ERR_ALLOC; }
+    p->mft_nb_cap = nb;
+    return FRESNEL_OK;
+}
+
+} // namespace
+
+extern "C" {
+
+fresnel_status fresnel_plan_reserve_mft(fresnel_plan *p, int nb_max)
+{
+    if (!p || nb_max <= 0 || nb_max > 8192) return FRESNEL_ERR_INVALID_ARG;
+    DeviceGuard g(p);
+    return mft_reserve(p, nb_max);
+}
+
+fresnel_status fresnel_mft(fresnel_plan *p, const void *in, void *out, int nb, const double *pixel_in, const double *pixel_out,
+                           const double *lambda, double f, int direction)
+{
+    if (!p || !in || !out || in == out || nb <= 0 || nb > 8192) return FRESNEL_ERR_INVALID_ARG;
+    if (!valid_positive(pixel_in, p->batch) || !valid_positive(pixel_out, p->batch) || !valid_positive(lambda, p->batch)) return FRESNEL_ERR_INVALID_ARG;
+    if (!std::isfinite(f) || f == 0.0 || (direction != FRESNEL_FORWARD && direction != FRESNEL_INVERSE)) return FRESNEL_ERR_INVALID_ARG;
+    DeviceGuard g(p);
+    fresnel_status st = mft_reserve(p, nb);
+    if (st != FRESNEL_OK) return st;
+    const int nbt = p->batch, na = p->N;
+    // per batch element: c = dx dx'/(lambda f) in turns (double-double), alpha = dx^2/(+- i lambda f) = -+ i dx^2/(lambda f)
+    std::vector<double> key(2 + 2 * (size_t)nbt), scal(4 * (size_t)nbt);
+    key[0] = nb; key[1] = direction;
+    for (int b = 0; b < nbt; ++b) {
+        const long double c = (long double)pixel_in[b] * (long double)pixel_out[b] / ((long double)lambda[b] * (long double)f);
+        const double hi = (double)c, lo = (double)(c - (long double)hi);
+        const double gq = (double)((long double)pixel_in[b] * (long double)pixel_in[b] / ((long double)lambda[b] * (long double)f));
+        key[2 + b] = hi; key[2 + nbt + b] = lo;
+        scal[b] = hi; scal[nbt + b] = lo; scal[2 * (size_t)nbt + b] = 0.0; scal[3 * (size_t)nbt + b] = direction == FRESNEL_FORWARD ? -gq : gq;
+    }
+    const bool cap = capture_state(p).active;
+    double2 *alpha = reinterpret_cast<double2 *>(p->mft_scal + 4 * (size_t)nbt);
+    for (int b0 = 0; b0 < nbt; b0 += 32) {                     // the scalars travel as kernel parameters
+        MftScalArgs a;
+        a.dst = p->mft_scal; a.batch = nbt; a.b0 = b0; a.n = nbt - b0 < 32 ? nbt - b0 : 32;
+        for (int r = 0; r < 4; ++r)
+            for (int i = 0; i < a.n; ++i) a.v[r][i] = scal[(size_t)r * nbt + b0 + i];
+        mft_scalars_kernel<<<1, 32, 0, p->stream>>>(a);
+        ++p->launches;
+    }
+    mft_alpha_kernel<<<(nbt + 127) / 128, 128, 0, p->stream>>>(p->mft_scal, alpha, nbt);
+    ++p->launches;
+    if (cap || p->mft_key != key) {                            // the kernel matrix of this geometry
+        MftMatrixArgs m;
+        m.out = p->mft_e; m.na = na; m.nb = nb; m.batch = nbt; m.sign = direction == FRESNEL_FORWARD ? -1 : +1;
+        m.c_hi = p->mft_scal; m.c_lo = p->mft_scal + nbt;
+        mft_matrix_kernel<<<dim3((na + 255) / 256, nb, nbt), 256, 0, p->stream>>>(m);
+        ++p->launches;
+        if (cap) p->mft_key.clear(); else p->mft_key = key;
+    }
+    if (cudaGetLastError() != cudaSuccess) return FRESNEL_ERR_CUDA;
+    // T^t[q,j] = sum_k U[j,k] E[q,k]
+    MftGemmArgs g1;
+    g1.A = in; g1.B = p->mft_e; g1.C = p->mft_t; g1.M = na; g1.N = nb; g1.K = na;
+    g1.strideA = (size_t)na * na; g1.strideB = (size_t)nb * na; g1.strideC = (size_t)nb * na; g1.alpha = nullptr;
+    cudaError_t e = p->dtype == FRESNEL_C128 ? launch_mft_gemm<double2, double2, true>(g1, nbt, p->stream)
+                                             : launch_mft_gemm<float2, double2, true>(g1, nbt, p->stream);
+    if (e != cudaSuccess) return FRESNEL_ERR_CUDA;
+    ++p->launches;
+    // V[p,q] = alpha sum_j E[p,j] T^t[q,j]
+    MftGemmArgs g2;
+    g2.A = p->mft_e; g2.B = p->mft_t; g2.C = out; g2.M = nb; g2.N = nb; g2.K = na;
+    g2.strideA = (size_t)nb * na; g2.strideB = (size_t)nb * na; g2.strideC = (size_t)nb * nb; g2.alpha = alpha;
+    e = p->dtype == FRESNEL_C128 ? launch_mft_gemm<double2, double2, false>(g2, nbt, p->stream)
+                                 : launch_mft_gemm<double2, float2, false>(g2, nbt, p->stream);
+    if (e != cudaSuccess) return FRESNEL_ERR_CUDA;
+    ++p->launches;
+    return FRESNEL_OK;
 }
 
 // ---- broadband image: incoherent sum over the batch ---------------------------------------------------------

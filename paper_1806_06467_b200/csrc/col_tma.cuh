@@ -126,7 +126,17 @@ col_tma_kernel(PassArgs<T> a, const __grid_constant__ CUtensorMap tmap, const __
     constexpr int TL = N / 16;                       // threads per column
     constexpr int ES = (int)sizeof(C);
     constexpr int ROW_BYTES = W * ES;
-    constexpr int GT = (W == 1) ? 0 : TL;            // group barrier size (W == 1: the CTA is the group)
+    // Thread <-> (column g, position j).  complex64: adjacent lanes take adjacent columns of the same row, so a warp reads
+    // and writes whole tile rows -- 8-byte elements of 16 / 32-byte rows otherwise cost two to four shared-memory wavefronts
+    // per access (ncu: ten times the bank conflicts of the row pass) -- at the price of CTA-wide exchange barriers instead of
+    // one named barrier per column group (measured: column pass -3..5 % at N = 2048..8192).  complex128 (16-byte elements,
+    // swizzled 32-byte rows) gains nothing from it and keeps one thread group per column.  FR_COL_INTERLEAVE: bit 0
+    // complex64, bit 1 complex128 (tuning builds).
+#ifndef FR_COL_INTERLEAVE
+#define FR_COL_INTERLEAVE 1
+#endif
+    constexpr bool IL = (W > 1) && (sizeof(T) == 4 ? (FR_COL_INTERLEAVE & 1) : (FR_COL_INTERLEAVE & 2)) != 0;
+    constexpr int GT = (W == 1 || IL) ? 0 : TL;      // group barrier size (0: the whole CTA)
     extern __shared__ __align__(1024) unsigned char fr_smem[];
     __shared__ __align__(8) uint64_t full_bar;
     __shared__ __align__(8) uint64_t map_bar;
@@ -136,8 +146,8 @@ col_tma_kernel(PassArgs<T> a, const __grid_constant__ CUtensorMap tmap, const __
     C *buf = reinterpret_cast<C *>(tile);
 
     const int tid = threadIdx.x;
-    const int g = tid / TL;                          // column of the tile == thread group
-    const int j = tid % TL;
+    const int g = IL ? tid % W : tid / TL;           // column of the tile (== thread group unless interleaved)
+    const int j = IL ? tid / W : tid % TL;
     const int b = blockIdx.y;
     const int col0 = blockIdx.x * W;
 
@@ -190,7 +200,7 @@ col_tma_kernel(PassArgs<T> a, const __grid_constant__ CUtensorMap tmap, const __
 #pragma unroll
         for (int r = 0; r < 16; ++r) v[r] = cmul(v[r], ldg_c(p + j + r * TL));
     }
-    line_transforms<T, N, MODE, false, W, GT>(v, buf, g, j, b, a, 1 + g, [&](C (&u)[16]) {
+    line_transforms<T, N, MODE, IL, W, GT>(v, buf, g, j, b, a, 1 + g, [&](C (&u)[16]) {
         // MODE_CONV2: the optic of the next surface on the resident tile; its maps arrive by TMA in the exchange
         // space, which is idle between the two convolutions
         using MT = MapTile<T, W>;

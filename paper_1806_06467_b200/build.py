@@ -59,6 +59,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if not force and os.path.exists(LIB) and os.path.exists(stamp) and open(stamp).read() == digest:
         return LIB
     jobs = [(os.path.join(CSRC, "fresnel_api.cu"), os.path.join(OBJ, "fresnel_api.o"), [])]
+    jobs.append((os.path.join(CSRC, "mr_inst.cu"), os.path.join(OBJ, "mr_inst.o"), []))
     for n in SIZES:
         jobs.append((os.path.join(CSRC, "pass_inst.cu"), os.path.join(OBJ, f"pass_{n}.o"), [f"-DFR_N={n}"]))
     with cf.ThreadPoolExecutor(max_workers=min(len(jobs), os.cpu_count() or 4)) as ex:

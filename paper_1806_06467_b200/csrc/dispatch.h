@@ -18,4 +18,11 @@ namespace fresnel {
     int col_tma_width_f64_##N();
 FR_DECL(64) FR_DECL(128) FR_DECL(256) FR_DECL(512) FR_DECL(1024) FR_DECL(2048) FR_DECL(4096) FR_DECL(8192)
 #undef FR_DECL
+
+// register-resident mixed-radix pass (mr_kernel.cuh, instantiated in mr_inst.cu) for these grid sizes
+#define FR_MR_SIZES(X) X(700) X(1400) X(2800)
+template <typename T> struct GenArgs;
+cudaError_t launch_mr_f32(int N, bool col, int mode, const GenArgs<float> &a, const CUtensorMap &m, int batch, cudaStream_t s);
+cudaError_t launch_mr_f64(int N, bool col, int mode, const GenArgs<double> &a, const CUtensorMap &m, int batch, cudaStream_t s);
+int mr_col_width(int N, int elem_bytes);
 } // namespace fresnel

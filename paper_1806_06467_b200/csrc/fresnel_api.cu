@@ -86,6 +86,7 @@ struct fresnel_plan {
     int gen_M = 0, gen_nstages = 0, gen_radix[kGenMaxStages] = {0};
     int gen_wcol = 1, gen_box_rows = 256;
     bool gen_tma = false;               // column tiles by TMA (needs a 16-byte multiple row pitch: not complex64 with odd N)
+    bool mr = false;                    // this N has a register-resident mixed-radix pass (mr_kernel.cuh)
     void *gen_tw = nullptr, *gen_blu_w = nullptr, *gen_blu_b = nullptr;
     // matrix Fourier transform (mft.cuh): kernel matrix E [batch][nb][N], intermediate T^t [batch][nb][N], per-batch scalars
     double2 *mft_e = nullptr, *mft_t = nullptr;
@@ -414,6 +415,12 @@ fresnel_status setup_generic(fresnel_plan *p)
     p->gen_tma = ((size_t)N * es) % 16 == 0 && std::getenv("FRESNEL_NO_TMA") == nullptr;
     p->generic = true;
     p->fuse = 0;
+    // selected sizes (2800 = 5*5*7*16, ...) have a register-resident pass; its column tiles are TMA tiles of its own width
+    const int wmr = mr_col_width(N, es);
+    if (wmr > 0 && p->gen_tma && std::getenv("FRESNEL_NO_MR") == nullptr) {
+        p->mr = true;
+        p->gen_wcol = wmr;
+    }
     return p->dtype == FRESNEL_C128 ? build_generic_tables<double2>(p, bluestein) : build_generic_tables<float2>(p, bluestein);
 }
 
@@ -473,7 +480,7 @@ bool make_tensor_map(fresnel_plan *p, void *wf)
     cuuint32_t box[3] = {(cuuint32_t)(2 * p->tma_w), p->generic ? (cuuint32_t)p->gen_box_rows : 256u, 1u};
     cuuint32_t estr[3] = {1, 1, 1};
     const size_t row_bytes = (size_t)p->tma_w * es;
-    CUtensorMapSwizzle sw = p->generic ? CU_TENSOR_MAP_SWIZZLE_NONE
+    CUtensorMapSwizzle sw = (p->generic && !p->mr) ? CU_TENSOR_MAP_SWIZZLE_NONE
                           : row_bytes == 32 ? CU_TENSOR_MAP_SWIZZLE_32B
                           : row_bytes == 64 ? CU_TENSOR_MAP_SWIZZLE_64B
                           : row_bytes == 128 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE;
@@ -545,6 +552,10 @@ template <typename T> cudaError_t run_generic(fresnel_plan *p, void *wf, const P
     a.pre = (const C *)q.pre; a.mid = (const C *)q.mid; a.rowfac = (const C *)q.rowfac;
     a.amp = (const T *)q.amp; a.opd = (const T *)q.opd; a.inv_lambda = q.inv_lambda;
     a.scale = (T)q.scale; a.pdl = p->pdl;
+    if (p->mr && (!q.col || tma)) {
+        if constexpr (sizeof(T) == 8) return launch_mr_f64(p->N, q.col, q.mode, a, p->tmap, p->batch, p->stream);
+        else return launch_mr_f32(p->N, q.col, q.mode, a, p->tmap, p->batch, p->stream);
+    }
     return launch_gen_pass<T>(a, p->tmap, p->batch, gen_smem(p, a.W), p->stream);
 }
 

@@ -1,8 +1,10 @@
 """Grids that are not a power of two ("N = 2800 ran faster than
 4096"; :259 npix = 1025), run with -m gpu.  The CUDA path (gen_kernel.cuh: mixed-radix Stockham stages in shared
-memory, Bluestein for sizes with a large prime factor) against the oracle's plain O(N^3) separable DFT, whole field,
-north-star tolerances + the max-abs bound.  Sizes: 100 = 2^2 5^2, 130 = 2 5 13, 175 = 5^2 7 (odd), 243 = 3^5 (odd),
-360 = 2^3 3^2 5, 1025 = 5^2 41 (odd, Bluestein over M = 2058), 1100 = 2^2 5^2 11, 2800 = 2^4 5^2 7.
+memory, Bluestein for sizes with a large prime factor; mr_kernel.cuh: the register-resident mixed-radix pass of
+N = 700, 1400, 2800) against the oracle's plain O(N^3) separable DFT, whole field, north-star tolerances + the max-abs
+bound.  Sizes: 100 = 2^2 5^2, 130 = 2 5 13, 175 = 5^2 7 (odd), 243 = 3^5 (odd), 360 = 2^3 3^2 5, 700 = 2^2 5^2 7
+(register-resident: partial butterfly rounds, a partial last TMA box), 1025 = 5^2 41 (odd, Bluestein over M = 2058),
+1100 = 2^2 5^2 11, 1400 = 2^3 5^2 7, 2800 = 2^4 5^2 7.
 """
 import math
 
@@ -13,7 +15,7 @@ from test_gpu_parity import TOL, assert_parity, field, map_dev, map_host, to_dev
 
 pytestmark = pytest.mark.gpu
 
-SIZES = [100, 130, 175, 243, 360, 1025]
+SIZES = [100, 130, 175, 243, 360, 700, 1025]
 
 
 @pytest.fixture(scope="module")
@@ -69,7 +71,7 @@ def test_propagate_as_and_direct_any_n(torch_cuda, B, oracle, N, dtype):
 
 
 @pytest.mark.parametrize("dtype", ["c128", "c64"])
-@pytest.mark.parametrize("N", [175, 360, 1025])
+@pytest.mark.parametrize("N", [175, 360, 700, 1025])
 def test_surface_and_train_any_n(torch_cuda, B, oracle, N, dtype):
     """The fused surface (lens + amplitude + OPD + angular spectrum), the stand-alone operators, the broadband image
     and a train with AUTO (a mix of angular spectrum and direct) on non-power-of-two grids."""
@@ -131,6 +133,33 @@ def test_n2800_the_papers_size(torch_cuda, B, oracle, dtype):
     want, dxo = oracle.propagate_direct(u[0], dx[0], lam[0], 0.5)
     assert px[0] == pytest.approx(dxo, rel=1e-15)
     assert_parity(d.cpu().numpy(), want[None], dtype)
+
+
+@pytest.mark.parametrize("dtype", ["c128", "c64"])
+def test_n1400_register_resident_all_modes(torch_cuda, B, oracle, dtype):
+    """N = 1400 = 5 * 5 * 7 * 8 on the register-resident mixed-radix pass (mr_kernel.cuh): inverse and centred transforms,
+    angular spectrum, direct Fresnel with z < 0, and a surface with both maps on the load of the row pass."""
+    from paper_1806_06467_b200 import inputs
+    N = 1400
+    u = field(N, 11500, 1, dtype)
+    dx, lam = np.array([1.5e-5]), np.array([0.8e-6])
+    zc = N * dx[0] ** 2 / lam[0]
+    plan = B.Plan(N, 1, dtype)
+    for direction, centered in ((-1, False), (+1, True)):
+        d = to_dev(torch_cuda, u, dtype)
+        plan.fft2d(d, direction, centered)
+        assert_parity(d.cpu().numpy(), oracle.fft2d(u[0], direction, centered)[None], dtype, f"fft2d {direction} {centered}")
+    d = to_dev(torch_cuda, u, dtype)
+    px = plan.propagate_direct(d, dx, lam, -1.2 * zc)
+    want, dxo = oracle.propagate_direct(u[0], dx[0], lam[0], -1.2 * zc)
+    assert px[0] == pytest.approx(dxo, rel=1e-15)
+    assert_parity(d.cpu().numpy(), want[None], dtype, "direct z < 0")
+    amp = inputs.circular_aperture(N, N / 3)
+    opd = inputs.psd_map(N, 1.5e-5, 3.0, 15e-9, 11501)
+    d = to_dev(torch_cuda, u, dtype)
+    plan.surface_as(d, dx, lam, 0.7, map_dev(torch_cuda, amp, dtype), map_dev(torch_cuda, opd, dtype), 0.2 * zc)
+    want = oracle.surface_as_batch(u, dx, lam, 0.7, map_host(amp, dtype), map_host(opd, dtype), 0.2 * zc)
+    assert_parity(d.cpu().numpy(), want, dtype, "surface")
 
 
 def test_n1100_radix_11_and_capacity_limits(torch_cuda, B, oracle):

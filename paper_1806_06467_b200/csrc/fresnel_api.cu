@@ -306,16 +306,41 @@ bool valid_positive(const double *v, int n)
 }
 
 // ---- grids that are not a power of two ---------------------------------------------------------------------------
-// Radices of a length-M mixed-radix transform (16, 8, 4, 2, then 13, 11, 7, 5, 3); false if M has another prime factor.
+// Radices of a length-M mixed-radix transform (16, 8, 4, 2, then 13, 11, 7, 5, 3); what is left may be ONE prime of
+// gen_prime() (17 .. 61), which then becomes the first stage (gen_stage_prime: a direct DFT without twiddles).  False if
+// M has any other prime factor.
 bool factor_radices(int M, int *radix, int *nstages)
 {
     int n = 0;
     auto take = [&](int r) {
-        while (M % r == 0 && n < kGenMaxStages) { radix[n++] = r; M /= r; }
+        while (M % r == 0 && n < kGenMaxStages - 1) { radix[n++] = r; M /= r; }
     };
     take(16); take(8); take(4); take(2); take(13); take(11); take(7); take(5); take(3);
+    if (M > 1 && gen_prime_offset(M) >= 0) {
+        for (int i = n; i > 0; --i) radix[i] = radix[i - 1];
+        radix[0] = M;
+        ++n;
+        M = 1;
+    }
     *nstages = n;
     return M == 1;
+}
+
+// cos / sin (2 pi m / P) of the primes 17 .. 61 into the constant memory of the current device (idempotent)
+fresnel_status upload_prime_roots()
+{
+    std::vector<double2> h(kGenPrimeRootsTotal);
+    int off = 0;
+    for (int i = 0; i < kGenNumPrimes; ++i) {
+        const int P = gen_prime(i);
+        for (int m = 0; m < P; ++m) {
+            const long double a = 2.0L * PI_L * (long double)m / (long double)P;
+            h[off + m].x = (double)cosl(a);
+            h[off + m].y = (double)sinl(a);
+        }
+        off += P;
+    }
+    return cudaMemcpyToSymbol(fr_prime_roots, h.data(), h.size() * sizeof(double2)) == cudaSuccess ? FRESNEL_OK : FRESNEL_ERR_CUDA;
 }
 
 int next_smooth(int m)      // smallest 7-smooth integer >= m
@@ -413,6 +438,10 @@ fresnel_status setup_generic(fresnel_plan *p)
     p->gen_wcol = (2 * gen_smem(p, wpref) <= (size_t)kGenMaxSmem) ? wpref : wmin;
     p->gen_box_rows = N < 256 ? N : 256;
     p->gen_tma = ((size_t)N * es) % 16 == 0 && std::getenv("FRESNEL_NO_TMA") == nullptr;
+    if (p->gen_radix[0] > 16) {
+        fresnel_status st = upload_prime_roots();
+        if (st != FRESNEL_OK) return st;
+    }
     p->generic = true;
     p->fuse = 0;
     // selected sizes (2800 = 5*5*7*16, ...) have a register-resident pass; its column tiles are TMA tiles of its own width

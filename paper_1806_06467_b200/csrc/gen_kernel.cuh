@@ -2,9 +2,12 @@
 //
 // The paper ran N = 2800 and found it faster than 4096; its App. B uses npix = 1025 (:259).
 // A line of N points (any N) lives in shared memory and is transformed there:
-//   * N = 2^a 3^b 5^c 7^d 11^e 13^f: mixed-radix Stockham stages (radix 16/8/4/2 from fft_core.cuh, odd radices
-//     in their symmetric form), ping-ponging between two line buffers; twiddles W_N^m come exactly rounded from
-//     one table of N entries (never by recurrence);
+//   * N = 2^a 3^b 5^c 7^d 11^e 13^f [x one prime P, 17 <= P <= 61]: mixed-radix Stockham stages (radix 16/8/4/2 from
+//     fft_core.cuh, odd radices in their symmetric form), ping-ponging between two line buffers; twiddles W_N^m come
+//     exactly rounded from one table of N entries (never by recurrence).  The larger prime (1025 = 5^2 41, and the
+//     paper's App. B grid npix = 1025 at beam ratio 0.25, N = 4100 = 2^2 5^2 41) is the FIRST stage
+//     -- no twiddles -- as a direct P-point DFT, a warp taking a block of outputs with the roots in constant memory
+//     (gen_stage_prime);
 //   * any other N (1025 = 5^2 41): Bluestein -- a length-N DFT is  chirp x circular convolution x chirp,
 //         X[k] = w[k] sum_n (x[n] w[n]) conj(w)[k-n],   w[n] = exp(-i pi n^2 / N),
 //     the convolution of length M >= 2N-1 (the next 7-smooth size) done by the same mixed-radix stages on the
@@ -50,6 +53,27 @@ template <typename T> struct GenArgs {
     T scale;
     int pdl;
 };
+
+// ---- one prime factor 17 <= P <= 61 as a direct DFT --------------------------------------------------------------
+// cos / sin (2 pi m / P), m = 0 .. P-1, of every such prime back to back, written once per device at plan creation
+// (long double on the host, rounded once).  Only the translation unit that owns the generic kernel fills and reads it.
+constexpr int kGenNumPrimes = 12;
+__host__ __device__ constexpr int gen_prime(int i)
+{
+    constexpr int primes[kGenNumPrimes] = {17, 19, 23, 29, 31, 37, 41, 43, 47, 53, 59, 61};
+    return primes[i];
+}
+__host__ __device__ constexpr int gen_prime_offset(int P)      // of its roots in fr_prime_roots; -1: not one of them
+{
+    int off = 0;
+    for (int i = 0; i < kGenNumPrimes; ++i) {
+        if (gen_prime(i) == P) return off;
+        off += gen_prime(i);
+    }
+    return -1;
+}
+constexpr int kGenPrimeRootsTotal = 460;      // sum of the primes
+static __constant__ double2 fr_prime_roots[kGenPrimeRootsTotal];
 
 // ---- odd-radix butterflies, symmetric form:  X[q], X[P-q] = (a0 + sum_t c_{tq} (a_t + a_{P-t})) -+ i (sum_t s_{tq} (a_t - a_{P-t}))
 // cos / sin of 2 pi i / P, i = 1 .. (P-1)/2, to 30 digits
@@ -170,6 +194,63 @@ FR_DEV void gen_stage(const typename cplx_of<T>::type *__restrict__ src, typenam
     }
 }
 
+// First stage (Ns = 1: no twiddles) of prime radix P > 16, dense src -> dst.  Symmetric form as in dft_odd, but the P
+// points do not fit the registers of one thread: a task is (block of QC output pairs, 32 butterflies); the warp that
+// takes it streams the input pairs x[t], x[P-t] from shared memory once and keeps 2 QC complex accumulators per lane; the
+// roots are warp-uniform reads of constant memory.  X[q], X[P-q] = (x0 + sum_t c_{tq} (x_t + x_{P-t})) -+ i (sum_t
+// s_{tq} (x_t - x_{P-t})).
+template <typename T, bool POUT>
+FR_DEV void gen_stage_prime(const typename cplx_of<T>::type *__restrict__ src, typename cplx_of<T>::type *__restrict__ dst, int len, int W,
+                            int P, int tid)
+{
+    using C = typename cplx_of<T>::type;
+    constexpr int QC = 8;
+    const int nb = len / P, H = (P - 1) / 2;
+    const int roff = gen_prime_offset(P);
+    const int items = nb * W, nblk = (items + 31) / 32, nchunk = (H + QC - 1) / QC;
+    const int warp = tid >> 5, lane = tid & 31;
+    for (int task = warp; task < nchunk * nblk; task += kGenThreads / 32) {
+        const int c = task / nblk, blk = task - c * nblk;
+        const int item = blk * 32 + lane;
+        if (item >= items) continue;
+        const int b = item / W, g = item - b * W;
+        const int q0 = c * QC + 1;                                  // this task's outputs: q0 .. q0 + QC - 1 (<= H) and P - q
+        const C x0 = src[(size_t)b * W + g];
+        C re[QC], im[QC], sum = x0;
+        int m[QC];
+#pragma unroll
+        for (int i = 0; i < QC; ++i) { re[i] = x0; im[i].x = (T)0; im[i].y = (T)0; m[i] = 0; }
+        for (int t = 1; t <= H; ++t) {
+            const C xa = src[(size_t)(b + t * nb) * W + g], xb = src[(size_t)(b + (P - t) * nb) * W + g];
+            const C sp = cadd(xa, xb), sm = csub(xa, xb);
+            sum = cadd(sum, sp);
+#pragma unroll
+            for (int i = 0; i < QC; ++i) {
+                m[i] += q0 + i;                                     // t q mod P
+                if (m[i] >= P) m[i] -= P;
+                const double2 r = fr_prime_roots[roff + m[i]];
+                const T cc = (T)r.x, ss = (T)r.y;
+                re[i].x += cc * sp.x; re[i].y += cc * sp.y;
+                im[i].x += ss * sm.x; im[i].y += ss * sm.y;
+            }
+        }
+        C *o = dst + g;
+        const int p0 = b * P;
+        if (c == 0) o[(size_t)gen_pos<POUT>(p0) * W] = sum;
+#pragma unroll
+        for (int i = 0; i < QC; ++i) {
+            const int q = q0 + i;
+            if (q <= H) {
+                C a, z;                                              // X[q] = re - i im ; X[P-q] = re + i im
+                a.x = re[i].x + im[i].y; a.y = re[i].y - im[i].x;
+                z.x = re[i].x - im[i].y; z.y = re[i].y + im[i].x;
+                o[(size_t)gen_pos<POUT>(p0 + q) * W] = a;
+                o[(size_t)gen_pos<POUT>(p0 + P - q) * W] = z;
+            }
+        }
+    }
+}
+
 template <typename T, int R>
 FR_DEV void gen_stage_any(const typename cplx_of<T>::type *src, typename cplx_of<T>::type *dst, int len, int W, int Ns,
                           const typename cplx_of<T>::type *__restrict__ tw, int tid, bool pin, bool pout)
@@ -196,7 +277,11 @@ FR_DEV void gen_fft(typename cplx_of<T>::type *&src, typename cplx_of<T>::type *
         case 5:  gen_stage_any<T, 5>(src, dst, a.M, a.W, Ns, a.tw, tid, pin, pout); break;
         case 7:  gen_stage_any<T, 7>(src, dst, a.M, a.W, Ns, a.tw, tid, pin, pout); break;
         case 11: gen_stage_any<T, 11>(src, dst, a.M, a.W, Ns, a.tw, tid, pin, pout); break;
-        default: gen_stage_any<T, 13>(src, dst, a.M, a.W, Ns, a.tw, tid, pin, pout); break;
+        case 13: gen_stage_any<T, 13>(src, dst, a.M, a.W, Ns, a.tw, tid, pin, pout); break;
+        default:                                                    // one prime 17 .. 61, always the first stage
+            if (pout) gen_stage_prime<T, true>(src, dst, a.M, a.W, R, tid);
+            else gen_stage_prime<T, false>(src, dst, a.M, a.W, R, tid);
+            break;
         }
         Ns *= R;
         __syncthreads();

@@ -2,9 +2,10 @@
 4096"; :259 npix = 1025), run with -m gpu.  The CUDA path (gen_kernel.cuh: mixed-radix Stockham stages in shared
 memory, Bluestein for sizes with a large prime factor; mr_kernel.cuh: the register-resident mixed-radix pass of
 N = 700, 1400, 2800) against the oracle's plain O(N^3) separable DFT, whole field, north-star tolerances + the max-abs
-bound.  Sizes: 100 = 2^2 5^2, 130 = 2 5 13, 175 = 5^2 7 (odd), 243 = 3^5 (odd), 360 = 2^3 3^2 5, 700 = 2^2 5^2 7
-(register-resident: partial butterfly rounds, a partial last TMA box), 1025 = 5^2 41 (odd, Bluestein over M = 2058),
-1100 = 2^2 5^2 11, 1400 = 2^3 5^2 7, 2800 = 2^4 5^2 7.
+bound.  Sizes: 100 = 2^2 5^2, 130 = 2 5 13, 175 = 5^2 7 (odd), 243 = 3^5 (odd), 335 = 5 67 (odd, Bluestein over
+M = 672), 360 = 2^3 3^2 5, 488 = 2^3 61 and 1025 = 5^2 41 (odd; one prime 17..61 as a direct first stage), 700 = 2^2 5^2 7
+(register-resident: partial butterfly rounds, a partial last TMA box), 1100 = 2^2 5^2 11, 1400 = 2^3 5^2 7,
+2800 = 2^4 5^2 7, 4100 = 2^2 5^2 41 (the paper's App. B call: npix = 1025 at beam ratio 0.25).
 """
 import math
 
@@ -15,7 +16,7 @@ from test_gpu_parity import TOL, assert_parity, field, map_dev, map_host, to_dev
 
 pytestmark = pytest.mark.gpu
 
-SIZES = [100, 130, 175, 243, 360, 700, 1025]
+SIZES = [100, 130, 175, 243, 335, 360, 488, 700, 1025]
 
 
 @pytest.fixture(scope="module")
@@ -71,7 +72,7 @@ def test_propagate_as_and_direct_any_n(torch_cuda, B, oracle, N, dtype):
 
 
 @pytest.mark.parametrize("dtype", ["c128", "c64"])
-@pytest.mark.parametrize("N", [175, 360, 700, 1025])
+@pytest.mark.parametrize("N", [175, 335, 360, 700, 1025])
 def test_surface_and_train_any_n(torch_cuda, B, oracle, N, dtype):
     """The fused surface (lens + amplitude + OPD + angular spectrum), the stand-alone operators, the broadband image
     and a train with AUTO (a mix of angular spectrum and direct) on non-power-of-two grids."""
@@ -162,6 +163,40 @@ def test_n1400_register_resident_all_modes(torch_cuda, B, oracle, dtype):
     assert_parity(d.cpu().numpy(), want, dtype, "surface")
 
 
+@pytest.mark.parametrize("dtype", ["c128", "c64"])
+def test_n4100_the_papers_appendix_b_grid(torch_cuda, B, oracle, dtype):
+    """N = 4100 = 41 * 4 * 5 * 5: `WFIRSTSPC(npix=1025)` at beam ratio 0.25.  The oracle's O(N^3)
+    transform takes minutes at this size, so: (a) the centred forward transform on a 15 x 15 subset of its outputs, each
+    computed one by one by the oracle's matrix Fourier transform (pinned to the centred FFT by P24 / P24b); (b) the inverse
+    transform undoes it; (c) angular spectrum at half the Talbot distance of a field with a 100-pixel period: the exact
+    half-period shift (P6), which fails for any error in the transfer function's frequency index."""
+    N = 4100
+    u = field(N, 11600, 1, dtype)
+    plan = B.Plan(N, 1, dtype)
+    d = to_dev(torch_cuda, u, dtype)
+    plan.fft2d(d, +1, True)
+    got = d.cpu().numpy()[0]
+    lam, f, dx = 1e-6, 1.0, 1e-5
+    nb, stride = 15, 257
+    v = oracle.mft(u[0], dx, nb, stride * lam * f / (N * dx), lam, f, +1) / (dx * dx / (1j * lam * f))
+    idx = N // 2 + (np.arange(nb) - nb // 2) * stride
+    scale = np.linalg.norm(got) / N                      # rms of the whole spectrum: the bar is relative to the field, not the subset
+    assert np.linalg.norm(got[np.ix_(idx, idx)] - v) / (nb * scale) <= TOL[dtype]
+    assert np.abs(got[np.ix_(idx, idx)] - v).max() <= 50 * TOL[dtype] * np.abs(got).max()
+    assert np.linalg.norm(got) == pytest.approx(N * np.linalg.norm(u[0]), rel=10 * TOL[dtype])   # Parseval
+    plan.fft2d(d, -1, True)
+    assert_parity(d.cpu().numpy(), u, dtype, "inverse of forward")
+    # Talbot: period 100 px, z_T = 2 d^2 / lambda; at z_T / 2 the field comes back shifted by half a period along both axes
+    per = 100
+    cell = field(per, 11601, 1, dtype)[0]
+    w = np.tile(cell, (N // per, N // per))[None]
+    dxs, lams = np.array([1e-5]), np.array([1e-6])
+    zt = 2 * (per * dxs[0]) ** 2 / lams[0]
+    d = to_dev(torch_cuda, w, dtype)
+    plan.propagate_as(d, dxs, lams, zt / 2)
+    assert_parity(d.cpu().numpy(), np.roll(w, (per // 2, per // 2), axis=(1, 2)), dtype, "half Talbot distance")
+
+
 def test_n1100_radix_11_and_capacity_limits(torch_cuda, B, oracle):
     """1100 = 2^2 5^2 11 exercises the radix-11 butterfly; sizes beyond the shared-memory capacity are refused."""
     import ctypes
@@ -172,5 +207,5 @@ def test_n1100_radix_11_and_capacity_limits(torch_cuda, B, oracle):
     plan.fft2d(d, +1, False)
     assert_parity(d.cpu().numpy(), oracle.fft2d(u[0], +1, False)[None], "c128")
     h = ctypes.c_void_p()
-    assert B.lib().fresnel_plan_create(ctypes.byref(h), 4100, 1, 1) == 2       # 2^2 5^2 41: Bluestein would need M >= 8199
+    assert B.lib().fresnel_plan_create(ctypes.byref(h), 4268, 1, 1) == 2       # 2^2 11 97: Bluestein would need M >= 8535
     assert B.lib().fresnel_plan_create(ctypes.byref(h), 7300, 1, 1) == 2

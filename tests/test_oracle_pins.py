@@ -696,6 +696,18 @@ def test_P24_mft_equals_the_centred_fft_at_critical_sampling(oracle):
     assert rel(oracle.apply_qpf(m, dxo, lam, z), d) <= 1e-12
 
 
+def test_P24b_mft_on_a_coarser_grid_samples_the_centred_fft(oracle):
+    """With an output pitch of s critical pixels the matrix transform lands on every s-th bin of the centred FFT around the
+    centre bin: how tests/test_gpu_any_n.py takes single outputs of a 4100^2 transform from the oracle."""
+    lam, f, dx = 0.8e-6, 0.7, 1.5e-5
+    for na, nb, s in ((100, 9, 7), (45, 5, 4)):
+        u = rnd(na, 245 + na)
+        full = dx * dx / (1j * lam * f) * oracle.fft2d(u, +1, True)
+        v = oracle.mft(u, dx, nb, s * lam * f / (na * dx), lam, f, +1)
+        idx = na // 2 + (np.arange(nb) - nb // 2) * s
+        assert rel(v, full[np.ix_(idx, idx)]) <= 1e-12
+
+
 def test_P25_mft_closed_forms(oracle):
     """Closed forms on an output grid the FFT cannot reach (nb != na, 3.7x finer than critical): the centre sample is
     sum(U) dx^2/(i lambda f) exactly; a uniform square aperture gives the product of two Dirichlet kernels; a shifted

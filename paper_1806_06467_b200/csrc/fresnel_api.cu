@@ -87,7 +87,7 @@ struct fresnel_plan {
     int gen_wcol = 1, gen_box_rows = 256;
     bool gen_tma = false;               // column tiles by TMA (needs a 16-byte multiple row pitch: not complex64 with odd N)
     bool mr = false;                    // this N has a register-resident mixed-radix pass (mr_kernel.cuh)
-    void *gen_tw = nullptr, *gen_blu_w = nullptr, *gen_blu_b = nullptr;
+    void *gen_tw = nullptr, *gen_blu_w = nullptr, *gen_blu_b = nullptr, *gen_prime_roots = nullptr;
     // matrix Fourier transform (mft.cuh): kernel matrix E [batch][nb][N], intermediate T^t [batch][nb][N], per-batch scalars
     double2 *mft_e = nullptr, *mft_t = nullptr;
     double *mft_scal = nullptr;         // [4][batch]: c_hi, c_lo, alpha.re, alpha.im  (alpha interleaved at +2*batch)
@@ -307,7 +307,7 @@ bool valid_positive(const double *v, int n)
 
 // ---- grids that are not a power of two ---------------------------------------------------------------------------
 // Radices of a length-M mixed-radix transform (16, 8, 4, 2, then 13, 11, 7, 5, 3); what is left may be ONE prime of
-// gen_prime() (17 .. 61), which then becomes the first stage (gen_stage_prime: a direct DFT without twiddles).  False if
+// 17 .. 61, which then becomes the first stage (gen_stage_prime: a direct DFT without twiddles).  False if
 // M has any other prime factor.
 bool factor_radices(int M, int *radix, int *nstages)
 {
@@ -316,7 +316,7 @@ bool factor_radices(int M, int *radix, int *nstages)
         while (M % r == 0 && n < kGenMaxStages - 1) { radix[n++] = r; M /= r; }
     };
     take(16); take(8); take(4); take(2); take(13); take(11); take(7); take(5); take(3);
-    if (M > 1 && gen_prime_offset(M) >= 0) {
+    if (M > 1 && gen_is_stage_prime(M)) {
         for (int i = n; i > 0; --i) radix[i] = radix[i - 1];
         radix[0] = M;
         ++n;
@@ -324,23 +324,6 @@ bool factor_radices(int M, int *radix, int *nstages)
     }
     *nstages = n;
     return M == 1;
-}
-
-// cos / sin (2 pi m / P) of the primes 17 .. 61 into the constant memory of the current device (idempotent)
-fresnel_status upload_prime_roots()
-{
-    std::vector<double2> h(kGenPrimeRootsTotal);
-    int off = 0;
-    for (int i = 0; i < kGenNumPrimes; ++i) {
-        const int P = gen_prime(i);
-        for (int m = 0; m < P; ++m) {
-            const long double a = 2.0L * PI_L * (long double)m / (long double)P;
-            h[off + m].x = (double)cosl(a);
-            h[off + m].y = (double)sinl(a);
-        }
-        off += P;
-    }
-    return cudaMemcpyToSymbol(fr_prime_roots, h.data(), h.size() * sizeof(double2)) == cudaSuccess ? FRESNEL_OK : FRESNEL_ERR_CUDA;
 }
 
 int next_smooth(int m)      // smallest 7-smooth integer >= m
@@ -415,11 +398,11 @@ bool generic_supported(int N, fresnel_dtype dt)
         if (!factor_radices(M, radix, &ns)) return false;
     }
     const size_t es = dt == FRESNEL_C128 ? 16 : 8;
-    return 2 * gen_buffer_bytes(M, (int)(16 / es), (int)es) + 1024 <= (size_t)kGenMaxSmem;
+    return 2 * gen_buffer_bytes(M, (int)(16 / es), (int)es) + 1024 + kGenPrimeTableBytes <= (size_t)kGenMaxSmem;
 }
 
 // Shared memory of the generic pass: two line buffers of M x W complex + alignment slack.
-size_t gen_smem(const fresnel_plan *p, int W) { return 2 * gen_buffer_bytes(p->gen_M, W, (int)p->esize()) + 1024; }
+size_t gen_smem(const fresnel_plan *p, int W) { return 2 * gen_buffer_bytes(p->gen_M, W, (int)p->esize()) + 1024 + kGenPrimeTableBytes; }
 
 fresnel_status setup_generic(fresnel_plan *p)
 {
@@ -438,8 +421,15 @@ fresnel_status setup_generic(fresnel_plan *p)
     p->gen_wcol = (2 * gen_smem(p, wpref) <= (size_t)kGenMaxSmem) ? wpref : wmin;
     p->gen_box_rows = N < 256 ? N : 256;
     p->gen_tma = ((size_t)N * es) % 16 == 0 && std::getenv("FRESNEL_NO_TMA") == nullptr;
-    if (p->gen_radix[0] > 16) {
-        fresnel_status st = upload_prime_roots();
+    if (p->gen_radix[0] > 16) {                                   // (cos, sin)(2 pi m / P) of the prime first stage
+        const int P = p->gen_radix[0];
+        std::vector<double2> h(P);
+        for (int m = 0; m < P; ++m) {
+            const long double a = 2.0L * PI_L * (long double)m / (long double)P;
+            h[m].x = (double)cosl(a);
+            h[m].y = (double)sinl(a);
+        }
+        fresnel_status st = upload_vec(&p->gen_prime_roots, h);
         if (st != FRESNEL_OK) return st;
     }
     p->generic = true;
@@ -578,6 +568,7 @@ template <typename T> cudaError_t run_generic(fresnel_plan *p, void *wf, const P
     a.nstages = p->gen_nstages;
     for (int i = 0; i < p->gen_nstages; ++i) a.radix[i] = p->gen_radix[i];
     a.tw = (const C *)p->gen_tw; a.blu_w = (const C *)p->gen_blu_w; a.blu_b = (const C *)p->gen_blu_b;
+    a.prime_roots = (const double2 *)p->gen_prime_roots;
     a.pre = (const C *)q.pre; a.mid = (const C *)q.mid; a.rowfac = (const C *)q.rowfac;
     a.amp = (const T *)q.amp; a.opd = (const T *)q.opd; a.inv_lambda = q.inv_lambda;
     a.scale = (T)q.scale; a.pdl = p->pdl;
@@ -1002,6 +993,7 @@ fresnel_status fresnel_plan_destroy(fresnel_plan *p)
         cudaFree(p->gen_tw);
         cudaFree(p->gen_blu_w);
         cudaFree(p->gen_blu_b);
+        cudaFree(p->gen_prime_roots);
         cudaFree(p->mft_e);
         cudaFree(p->mft_t);
         cudaFree(p->mft_scal);

@@ -26,7 +26,7 @@
 namespace fresnel {
 
 constexpr int kGenMaxStages = 14;
-constexpr int kGenThreads = 256;
+constexpr int kGenThreads = 256;          // CTA size where two CTAs fit an SM; 2 * kGenThreads where only one does
 constexpr int kGenMaxSmem = 226 * 1024;   // dynamic shared memory the generic pass may ask for (227 KB minus its static part)
 
 // bytes of one line buffer (M x W complex), rounded up to the 128-byte alignment TMA wants of a shared-memory box
@@ -45,6 +45,7 @@ template <typename T> struct GenArgs {
     int nstages;
     int radix[kGenMaxStages]; // of the length-M transform, in order
     const C *tw;              // [M] forward roots W_M^m = exp(-2 pi i m / M)
+    const double2 *prime_roots; // [P] (cos, sin)(2 pi m / P) of the first stage's prime radix P > 16, or nullptr
     const C *blu_w;           // [N] Bluestein chirp exp(-i pi n^2 / N) or nullptr (mixed radix)
     const C *blu_b;           // [M] transform of the chirp filter, scaled by 1/M
     const C *pre, *mid, *rowfac;      // [batch][N] tables as in PassArgs
@@ -54,26 +55,16 @@ template <typename T> struct GenArgs {
     int pdl;
 };
 
-// ---- one prime factor 17 <= P <= 61 as a direct DFT --------------------------------------------------------------
-// cos / sin (2 pi m / P), m = 0 .. P-1, of every such prime back to back, written once per device at plan creation
-// (long double on the host, rounded once).  Only the translation unit that owns the generic kernel fills and reads it.
-constexpr int kGenNumPrimes = 12;
-__host__ __device__ constexpr int gen_prime(int i)
+// ---- one prime factor 17 <= P <= 61 as a direct DFT (gen_stage_prime) ---------------------------------------------
+constexpr int kGenMaxPrime = 61;
+__host__ __device__ constexpr bool gen_is_stage_prime(int P)
 {
-    constexpr int primes[kGenNumPrimes] = {17, 19, 23, 29, 31, 37, 41, 43, 47, 53, 59, 61};
-    return primes[i];
+    if (P < 17 || P > kGenMaxPrime) return false;
+    for (int d = 2; d * d <= P; ++d)
+        if (P % d == 0) return false;
+    return true;
 }
-__host__ __device__ constexpr int gen_prime_offset(int P)      // of its roots in fr_prime_roots; -1: not one of them
-{
-    int off = 0;
-    for (int i = 0; i < kGenNumPrimes; ++i) {
-        if (gen_prime(i) == P) return off;
-        off += gen_prime(i);
-    }
-    return -1;
-}
-constexpr int kGenPrimeRootsTotal = 460;      // sum of the primes
-static __constant__ double2 fr_prime_roots[kGenPrimeRootsTotal];
+constexpr size_t kGenPrimeTableBytes = 1024;   // shared-memory copy of the roots behind the two line buffers (61 x 16 bytes)
 
 // ---- odd-radix butterflies, symmetric form:  X[q], X[P-q] = (a0 + sum_t c_{tq} (a_t + a_{P-t})) -+ i (sum_t s_{tq} (a_t - a_{P-t}))
 // cos / sin of 2 pi i / P, i = 1 .. (P-1)/2, to 30 digits
@@ -165,7 +156,7 @@ FR_DEV void gen_stage(const typename cplx_of<T>::type *__restrict__ src, typenam
     using C = typename cplx_of<T>::type;
     const int nb = len / R;                    // butterflies per line
     const int tstep = len / (Ns * R);          // W_{Ns R}^{t k} = W_len^{t k tstep}
-    for (int idx = tid; idx < nb * W; idx += kGenThreads) {
+    for (int idx = tid; idx < nb * W; idx += (int)blockDim.x) {
         const int b = idx / W, g = idx - b * W;
         const int k = b % Ns;
         C v[R];
@@ -197,19 +188,18 @@ FR_DEV void gen_stage(const typename cplx_of<T>::type *__restrict__ src, typenam
 // First stage (Ns = 1: no twiddles) of prime radix P > 16, dense src -> dst.  Symmetric form as in dft_odd, but the P
 // points do not fit the registers of one thread: a task is (block of QC output pairs, 32 butterflies); the warp that
 // takes it streams the input pairs x[t], x[P-t] from shared memory once and keeps 2 QC complex accumulators per lane; the
-// roots are warp-uniform reads of constant memory.  X[q], X[P-q] = (x0 + sum_t c_{tq} (x_t + x_{P-t})) -+ i (sum_t
+// roots (cos, sin)(2 pi m / P) sit in shared memory and every read of them is one address per warp.  X[q], X[P-q] = (x0 + sum_t c_{tq} (x_t + x_{P-t})) -+ i (sum_t
 // s_{tq} (x_t - x_{P-t})).
 template <typename T, bool POUT>
 FR_DEV void gen_stage_prime(const typename cplx_of<T>::type *__restrict__ src, typename cplx_of<T>::type *__restrict__ dst, int len, int W,
-                            int P, int tid)
+                            int P, const double2 *roots, int tid)
 {
     using C = typename cplx_of<T>::type;
-    constexpr int QC = 8;
+    constexpr int QC = 5;                                           // P = 41: 4 blocks of 5 output pairs
     const int nb = len / P, H = (P - 1) / 2;
-    const int roff = gen_prime_offset(P);
     const int items = nb * W, nblk = (items + 31) / 32, nchunk = (H + QC - 1) / QC;
     const int warp = tid >> 5, lane = tid & 31;
-    for (int task = warp; task < nchunk * nblk; task += kGenThreads / 32) {
+    for (int task = warp; task < nchunk * nblk; task += (int)blockDim.x / 32) {
         const int c = task / nblk, blk = task - c * nblk;
         const int item = blk * 32 + lane;
         if (item >= items) continue;
@@ -228,7 +218,7 @@ FR_DEV void gen_stage_prime(const typename cplx_of<T>::type *__restrict__ src, t
             for (int i = 0; i < QC; ++i) {
                 m[i] += q0 + i;                                     // t q mod P
                 if (m[i] >= P) m[i] -= P;
-                const double2 r = fr_prime_roots[roff + m[i]];
+                const double2 r = roots[m[i]];                      // shared memory, one address per warp: a broadcast
                 const T cc = (T)r.x, ss = (T)r.y;
                 re[i].x += cc * sp.x; re[i].y += cc * sp.y;
                 im[i].x += ss * sm.x; im[i].y += ss * sm.y;
@@ -261,7 +251,7 @@ FR_DEV void gen_stage_any(const typename cplx_of<T>::type *src, typename cplx_of
 
 // forward transform of length len = a.M on the W lines in *src; on return *src holds the result (buffers swapped as needed)
 template <typename T>
-FR_DEV void gen_fft(typename cplx_of<T>::type *&src, typename cplx_of<T>::type *&dst, const GenArgs<T> &a, int tid)
+FR_DEV void gen_fft(typename cplx_of<T>::type *&src, typename cplx_of<T>::type *&dst, const GenArgs<T> &a, const double2 *roots, int tid)
 {
     using C = typename cplx_of<T>::type;
     int Ns = 1;
@@ -279,8 +269,8 @@ FR_DEV void gen_fft(typename cplx_of<T>::type *&src, typename cplx_of<T>::type *
         case 11: gen_stage_any<T, 11>(src, dst, a.M, a.W, Ns, a.tw, tid, pin, pout); break;
         case 13: gen_stage_any<T, 13>(src, dst, a.M, a.W, Ns, a.tw, tid, pin, pout); break;
         default:                                                    // one prime 17 .. 61, always the first stage
-            if (pout) gen_stage_prime<T, true>(src, dst, a.M, a.W, R, tid);
-            else gen_stage_prime<T, false>(src, dst, a.M, a.W, R, tid);
+            if (pout) gen_stage_prime<T, true>(src, dst, a.M, a.W, R, roots, tid);
+            else gen_stage_prime<T, false>(src, dst, a.M, a.W, R, roots, tid);
             break;
         }
         Ns *= R;
@@ -294,15 +284,15 @@ FR_DEV void gen_fft(typename cplx_of<T>::type *&src, typename cplx_of<T>::type *
 //   the chirp multiply; in the mixed-radix case the CALLER conjugates inside its neighbouring pointwise step.
 // Mixed radix: the transform itself.  Bluestein: chirp, zero-pad, FFT_M, x filter, inverse FFT_M, chirp.
 template <typename T>
-FR_DEV void gen_dft(typename cplx_of<T>::type *&src, typename cplx_of<T>::type *&dst, const GenArgs<T> &a, int tid, bool conj_in)
+FR_DEV void gen_dft(typename cplx_of<T>::type *&src, typename cplx_of<T>::type *&dst, const GenArgs<T> &a, const double2 *roots, int tid, bool conj_in)
 {
     using C = typename cplx_of<T>::type;
     const int N = a.N, M = a.M, W = a.W;
     if (a.blu_w == nullptr) {            // mixed radix: the caller has folded the conjugation into its own pointwise step
-        gen_fft<T>(src, dst, a, tid);
+        gen_fft<T>(src, dst, a, roots, tid);
         return;
     }
-    for (int e = tid; e < M * W; e += kGenThreads) {
+    for (int e = tid; e < M * W; e += (int)blockDim.x) {
         const int n = e / W;
         C x;
         x.x = (T)0; x.y = (T)0;
@@ -314,14 +304,14 @@ FR_DEV void gen_dft(typename cplx_of<T>::type *&src, typename cplx_of<T>::type *
         src[e] = x;
     }
     __syncthreads();
-    gen_fft<T>(src, dst, a, tid);
-    for (int e = tid; e < M * W; e += kGenThreads) {          // x filter, conjugate: inverse FFT_M = conj o FFT_M o conj
+    gen_fft<T>(src, dst, a, roots, tid);
+    for (int e = tid; e < M * W; e += (int)blockDim.x) {          // x filter, conjugate: inverse FFT_M = conj o FFT_M o conj
         const C t = cmul(src[e], ldg_c(a.blu_b + e / W));
         src[e].x = t.x; src[e].y = -t.y;
     }
     __syncthreads();
-    gen_fft<T>(src, dst, a, tid);
-    for (int e = tid; e < N * W; e += kGenThreads) {
+    gen_fft<T>(src, dst, a, roots, tid);
+    for (int e = tid; e < N * W; e += (int)blockDim.x) {
         C t = src[e];
         t.y = -t.y;
         src[e] = cmul(t, ldg_c(a.blu_w + e / W));
@@ -329,8 +319,8 @@ FR_DEV void gen_dft(typename cplx_of<T>::type *&src, typename cplx_of<T>::type *
     __syncthreads();
 }
 
-template <typename T>
-__global__ void __launch_bounds__(kGenThreads, 2) gen_pass_kernel(GenArgs<T> a, const __grid_constant__ CUtensorMap tmap)
+template <typename T, int NT>
+__global__ void __launch_bounds__(NT, NT == kGenThreads ? 2 : 1) gen_pass_kernel(GenArgs<T> a, const __grid_constant__ CUtensorMap tmap)
 {
     using C = typename cplx_of<T>::type;
     constexpr int ES = (int)sizeof(C);
@@ -340,6 +330,9 @@ __global__ void __launch_bounds__(kGenThreads, 2) gen_pass_kernel(GenArgs<T> a, 
     const int N = a.N, M = a.M, W = a.W;
     C *src = reinterpret_cast<C *>(base);
     C *dst = reinterpret_cast<C *>(base + gen_buffer_bytes(M, W, ES));     // 128-byte aligned: either buffer may feed the TMA store
+    const double2 *roots = reinterpret_cast<const double2 *>(base + 2 * gen_buffer_bytes(M, W, ES));
+    if (a.prime_roots != nullptr)                           // visible after the barriers that follow the load
+        for (int m = threadIdx.x; m < a.radix[0]; m += (int)blockDim.x) const_cast<double2 *>(roots)[m] = a.prime_roots[m];
     const int tid = threadIdx.x;
     const int b = blockIdx.y;
     const int line0 = blockIdx.x * W;                       // first row / column of this CTA
@@ -361,7 +354,7 @@ __global__ void __launch_bounds__(kGenThreads, 2) gen_pass_kernel(GenArgs<T> a, 
         mbar_wait(&full_bar, 0);
     } else if (a.col == 2) {
         const C *g0 = a.wf + (size_t)b * N * N + line0;
-        for (int e = tid; e < N * W; e += kGenThreads) {
+        for (int e = tid; e < N * W; e += (int)blockDim.x) {
             const int n = e / W, g = e - n * W;
             C x;
             x.x = (T)0; x.y = (T)0;
@@ -371,7 +364,7 @@ __global__ void __launch_bounds__(kGenThreads, 2) gen_pass_kernel(GenArgs<T> a, 
     } else {
         for (int g = 0; g < W; ++g) {
             const C *row = a.wf + (size_t)b * N * N + (size_t)(line0 + g) * N;
-            for (int n = tid; n < N; n += kGenThreads) {
+            for (int n = tid; n < N; n += (int)blockDim.x) {
                 C x;
                 x.x = (T)0; x.y = (T)0;
                 if (g < nl) {
@@ -388,7 +381,7 @@ __global__ void __launch_bounds__(kGenThreads, 2) gen_pass_kernel(GenArgs<T> a, 
     const bool inv = a.mode == MODE_INV, conv = a.mode == MODE_CONV, blu = a.blu_w != nullptr;
     if (a.pre != nullptr || (inv && !blu)) {
         const C *p = a.pre != nullptr ? a.pre + (size_t)b * N : nullptr;
-        for (int e = tid; e < N * W; e += kGenThreads) {
+        for (int e = tid; e < N * W; e += (int)blockDim.x) {
             C x = src[e];
             if (p != nullptr) x = cmul(x, ldg_c(p + e / W));
             if (inv && !blu) x.y = -x.y;
@@ -397,11 +390,11 @@ __global__ void __launch_bounds__(kGenThreads, 2) gen_pass_kernel(GenArgs<T> a, 
     }
     __syncthreads();
 
-    gen_dft<T>(src, dst, a, tid, inv && blu);                // F (or conj . F . with the closing conj below)
+    gen_dft<T>(src, dst, a, roots, tid, inv && blu);                // F (or conj . F . with the closing conj below)
     {
         const C *m = a.mid != nullptr ? a.mid + (size_t)b * N : nullptr;
         if (inv || m != nullptr || (conv && !blu)) {
-            for (int e = tid; e < N * W; e += kGenThreads) {
+            for (int e = tid; e < N * W; e += (int)blockDim.x) {
                 C x = src[e];
                 if (inv) x.y = -x.y;                         // closes the inverse transform
                 if (m != nullptr) x = cmul(x, ldg_c(m + e / W));
@@ -410,13 +403,13 @@ __global__ void __launch_bounds__(kGenThreads, 2) gen_pass_kernel(GenArgs<T> a, 
             }
             __syncthreads();
         }
-        if (conv) gen_dft<T>(src, dst, a, tid, blu);         // inverse transform = conj . F . conj (closing conj: on the store)
+        if (conv) gen_dft<T>(src, dst, a, roots, tid, blu);         // inverse transform = conj . F . conj (closing conj: on the store)
     }
     // ---- scale, per-row factor, store ----
     const T sx = a.scale, sy = conv ? -a.scale : a.scale;   // scale, and the closing conjugation of the convolution
     if (a.col == 1) {
         if (a.scale != (T)1 || conv)
-            for (int e = tid; e < N * W; e += kGenThreads) { src[e].x *= sx; src[e].y *= sy; }
+            for (int e = tid; e < N * W; e += (int)blockDim.x) { src[e].x *= sx; src[e].y *= sy; }
         fence_async_proxy();
         __syncthreads();
         if (tid == 0) {
@@ -425,7 +418,7 @@ __global__ void __launch_bounds__(kGenThreads, 2) gen_pass_kernel(GenArgs<T> a, 
         }
     } else if (a.col == 2) {
         C *g0 = a.wf + (size_t)b * N * N + line0;
-        for (int e = tid; e < N * W; e += kGenThreads) {
+        for (int e = tid; e < N * W; e += (int)blockDim.x) {
             const int n = e / W, g = e - n * W;
             if (g < nl) { C x = src[e]; x.x *= sx; x.y *= sy; g0[(size_t)n * N + g] = x; }
         }
@@ -438,7 +431,7 @@ __global__ void __launch_bounds__(kGenThreads, 2) gen_pass_kernel(GenArgs<T> a, 
                 const C c = ldg_c(a.rowfac + (size_t)b * N + line0 + g);
                 rf.x = c.x * a.scale; rf.y = c.y * a.scale;
             }
-            for (int n = tid; n < N; n += kGenThreads) {
+            for (int n = tid; n < N; n += (int)blockDim.x) {
                 C x = src[(size_t)n * W + g];
                 if (conv) x.y = -x.y;
                 row[n] = cmul(x, rf);
@@ -450,15 +443,18 @@ __global__ void __launch_bounds__(kGenThreads, 2) gen_pass_kernel(GenArgs<T> a, 
 template <typename T>
 cudaError_t launch_gen_pass(const GenArgs<T> &a, const CUtensorMap &tmap, int batch, size_t smem, cudaStream_t stream)
 {
-    auto kern = gen_pass_kernel<T>;
+    // two CTAs of kGenThreads per SM where their buffers fit, else one of twice the size
+    const bool two = 2 * (smem + 1024) <= (size_t)227 * 1024;
+    auto kern = two ? gen_pass_kernel<T, kGenThreads> : gen_pass_kernel<T, 2 * kGenThreads>;
     static std::atomic<unsigned long long> configured{0};
     if (fr_needs_configuring(configured)) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kGenMaxSmem);
+        cudaError_t e = cudaFuncSetAttribute(gen_pass_kernel<T, kGenThreads>, cudaFuncAttributeMaxDynamicSharedMemorySize, kGenMaxSmem);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(gen_pass_kernel<T, 2 * kGenThreads>, cudaFuncAttributeMaxDynamicSharedMemorySize, kGenMaxSmem);
         if (e != cudaSuccess) return e;
         fr_mark_configured(configured);
     }
     dim3 grid((a.N + a.W - 1) / a.W, batch, 1);
-    return launch_pdl(kern, grid, dim3(kGenThreads), smem, stream, a.pdl != 0, a, tmap);
+    return launch_pdl(kern, grid, dim3(two ? kGenThreads : 2 * kGenThreads), smem, stream, a.pdl != 0, a, tmap);
 }
 
 } // namespace fresnel

@@ -264,26 +264,31 @@ col_tma_kernel(PassArgs<T> a, const __grid_constant__ CUtensorMap tmap, const __
     }
 }
 
-// columns per tile for the TMA column pass
-__host__ __device__ constexpr int fr_tma_cols(int N, int elem_bytes)
+// columns per tile for the TMA column pass.  The fused pass (conv2: two convolutions and an optic per tile, i.e. twice the
+// arithmetic per byte) at N = 2048 does better with 16-byte-wide tiles and FOUR resident CTAs of one column group each than
+// with 32-byte-wide tiles and two CTAs (measured: 93.2 -> 86.2 us complex128, 57.3 -> 52.3 us complex64; the single
+// convolution is the other way round, 44.8 vs 48.4 us): the tile load of one CTA hides under three others.
+__host__ __device__ constexpr int fr_tma_cols(int N, int elem_bytes, bool conv2 = false)
 {
     const int TL = N / 16;
     if (elem_bytes == 16) {
 #ifdef FR_TMAW_F64
         if (FR_TMAW_F64 * TL <= 512) return FR_TMAW_F64;
 #endif
+        if (conv2 && N == 2048) return 1;
         return N <= 1024 ? 4 : (N <= 2048 ? 2 : 1);       // >= 2 resident CTAs per SM wherever the tile allows
     }
 #ifdef FR_TMAW_F32
     if (FR_TMAW_F32 * TL <= 1024) return FR_TMAW_F32;
 #endif
+    if (conv2 && N == 2048) return 2;
     return N <= 1024 ? 8 : (N <= 2048 ? 4 : 2);
 }
 
-template <typename T, int N> struct ColTmaGeom {
+template <typename T, int N, bool CONV2 = false> struct ColTmaGeom {
     static constexpr int TL = N / 16;
     static constexpr int ES = (int)sizeof(typename cplx_of<T>::type);
-    static constexpr int W = fr_tma_cols(N, ES);
+    static constexpr int W = fr_tma_cols(N, ES, CONV2);
     static constexpr int threads = W * TL;
     static constexpr size_t smem = (size_t)W * fr_padded_len(N) * ES;
     static constexpr int regs_goal = sizeof(T) == 8 ? FR_REGS_F64 : FR_REGS_F32;
@@ -303,7 +308,7 @@ template <typename T, int N, int MODE>
 cudaError_t launch_col_tma(const PassArgs<T> &a, const CUtensorMap &tmap, const CUtensorMap &tmap_amp2, const CUtensorMap &tmap_opd2,
                            int batch, cudaStream_t stream)
 {
-    using G = ColTmaGeom<T, N>;
+    using G = ColTmaGeom<T, N, MODE == MODE_CONV2>;
     if constexpr (!G::supported) {
         return cudaErrorNotSupported;
     } else {

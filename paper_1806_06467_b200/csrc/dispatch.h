@@ -14,8 +14,8 @@ namespace fresnel {
                                        const CUtensorMap &mo, int batch, cudaStream_t s);                                       \
     int col_tma_map_box_f32_##N();                                                                              \
     int col_tma_map_box_f64_##N();                                                                              \
-    int col_tma_width_f32_##N();                                                                                \
-    int col_tma_width_f64_##N();
+    int col_tma_width_f32_##N(bool conv2);                                                                      \
+    int col_tma_width_f64_##N(bool conv2);
 FR_DECL(64) FR_DECL(128) FR_DECL(256) FR_DECL(512) FR_DECL(1024) FR_DECL(2048) FR_DECL(4096) FR_DECL(8192)
 #undef FR_DECL
 

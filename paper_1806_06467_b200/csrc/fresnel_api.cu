@@ -77,6 +77,7 @@ struct fresnel_plan {
     unsigned long long launches = 0;
     int prefetch = 0;                   // L2 prefetch distance in tiles (see pass_kernel.cuh)
     int tma_w = 0;                      // columns per TMA tile of the column pass (0: not used for this N)
+    int tma_w2 = 0;                     // the same for the fused column pass (MODE_CONV2), which may prefer narrower tiles
     int map_box = 0;                    // columns per TMA box of a surface map (fused column pass)
     int sms = 148;
     int pdl = 1;                        // programmatic dependent launch of the pass kernels (FRESNEL_PDL=0: off, A/B timing)
@@ -95,6 +96,8 @@ struct fresnel_plan {
     std::vector<double> mft_key;        // what mft_e currently holds (nb, direction, c_hi.., c_lo..); empty: nothing
     CUtensorMap tmap{};                  // tensor map of the wavefront last seen by the column pass
     const void *tmap_wf = nullptr;
+    CUtensorMap tmap2;                  // wavefront tiles of the fused column pass
+    const void *tmap2_wf = nullptr;
     std::vector<MapDesc> map_descs;     // tensor maps of surface maps, by pointer
     cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};   // profiling hook, see fresnel_plan_record_pass_events
     bool ev_armed = false;
@@ -465,10 +468,10 @@ EncodeTiledFn encode_tiled_fn()
     return fn;
 }
 
-int query_tma_width(int N, fresnel_dtype dt)
+int query_tma_width(int N, fresnel_dtype dt, bool conv2)
 {
     switch (N) {
-#define FR_CASE(NN) case NN: return dt == FRESNEL_C128 ? col_tma_width_f64_##NN() : col_tma_width_f32_##NN();
+#define FR_CASE(NN) case NN: return dt == FRESNEL_C128 ? col_tma_width_f64_##NN(conv2) : col_tma_width_f32_##NN(conv2);
         FR_CASE(64) FR_CASE(128) FR_CASE(256) FR_CASE(512) FR_CASE(1024) FR_CASE(2048) FR_CASE(4096) FR_CASE(8192)
 #undef FR_CASE
     }
@@ -486,9 +489,16 @@ int query_map_box(int N, fresnel_dtype dt)
 }
 
 // The wavefront as a 3-D tensor {2N scalars, N rows, batch}; a box is {2W scalars, 256 rows, 1}.
-bool make_tensor_map(fresnel_plan *p, void *wf)
+bool make_tensor_map(fresnel_plan *p, void *wf, bool conv2 = false)
 {
-    if (p->tmap_wf == wf) return true;
+    const int tma_w = conv2 ? p->tma_w2 : p->tma_w;
+    if (conv2 && tma_w == p->tma_w) {                     // same tile geometry: one tensor map serves both
+        if (!make_tensor_map(p, wf, false)) return false;
+        p->tmap2 = p->tmap;
+        p->tmap2_wf = wf;
+        return true;
+    }
+    if ((conv2 ? p->tmap2_wf : p->tmap_wf) == wf) return true;
     EncodeTiledFn fn = encode_tiled_fn();
     if (!fn) return false;
     const bool dbl = p->dtype == FRESNEL_C128;
@@ -496,17 +506,18 @@ bool make_tensor_map(fresnel_plan *p, void *wf)
     const cuuint64_t N = (cuuint64_t)p->N;
     cuuint64_t gdim[3] = {2 * N, N, (cuuint64_t)p->batch};
     cuuint64_t gstr[2] = {N * es, N * N * es};
-    cuuint32_t box[3] = {(cuuint32_t)(2 * p->tma_w), p->generic ? (cuuint32_t)p->gen_box_rows : 256u, 1u};
+    cuuint32_t box[3] = {(cuuint32_t)(2 * tma_w), p->generic ? (cuuint32_t)p->gen_box_rows : 256u, 1u};
     cuuint32_t estr[3] = {1, 1, 1};
-    const size_t row_bytes = (size_t)p->tma_w * es;
+    const size_t row_bytes = (size_t)tma_w * es;
     CUtensorMapSwizzle sw = (p->generic && !p->mr) ? CU_TENSOR_MAP_SWIZZLE_NONE
                           : row_bytes == 32 ? CU_TENSOR_MAP_SWIZZLE_32B
                           : row_bytes == 64 ? CU_TENSOR_MAP_SWIZZLE_64B
                           : row_bytes == 128 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE;
-    CUresult r = fn(&p->tmap, dbl ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, wf, gdim, gstr, box, estr,
-                    CU_TENSOR_MAP_INTERLEAVE_NONE, sw, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    CUresult r = fn(conv2 ? &p->tmap2 : &p->tmap, dbl ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, wf, gdim,
+                    gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, sw, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) return false;
-    p->tmap_wf = wf;
+    (conv2 ? p->tmap2_wf : p->tmap_wf) = wf;
     return true;
 }
 
@@ -588,8 +599,10 @@ fresnel_status run_pass(fresnel_plan *p, void *wf, const PassSpec &q)
         ++p->launches;
         return FRESNEL_OK;
     }
-    const bool tma = q.col && p->tma_w > 0 && make_tensor_map(p, wf);
-    const CUtensorMap *ma = &p->tmap, *mo = &p->tmap;
+    const bool conv2 = q.mode == MODE_CONV2;
+    const bool tma = q.col && p->tma_w > 0 && make_tensor_map(p, wf, conv2);
+    const CUtensorMap &wmap = conv2 ? p->tmap2 : p->tmap;
+    const CUtensorMap *ma = &wmap, *mo = &wmap;
     if (tma && q.mode == MODE_CONV2) {
         if (q.amp2 && !(ma = map_tensor_map(p, q.amp2))) return FRESNEL_ERR_CUDA;
         if (q.opd2 && !(mo = map_tensor_map(p, q.opd2))) return FRESNEL_ERR_CUDA;
@@ -606,7 +619,7 @@ fresnel_status run_pass(fresnel_plan *p, void *wf, const PassSpec &q)
         a.inv_lambda = q.inv_lambda; a.scale = q.scale; a.prefetch_distance = prefetch; a.pdl = p->pdl;
         a.lens2 = (const double2 *)q.lens2; a.mid2 = (const double2 *)q.mid2; a.amp2 = (const double *)q.amp2; a.opd2 = (const double *)q.opd2;
         switch (p->N) {
-#define FR_CASE(NN) case NN: e = tma ? launch_col_tma_f64_##NN(q.mode, a, p->tmap, *ma, *mo, p->batch, p->stream)           \
+#define FR_CASE(NN) case NN: e = tma ? launch_col_tma_f64_##NN(q.mode, a, wmap, *ma, *mo, p->batch, p->stream)           \
                                    : launch_pass_f64_##NN(q.col, q.mode, a, p->batch, p->stream); break;
             FR_CASE(64) FR_CASE(128) FR_CASE(256) FR_CASE(512) FR_CASE(1024) FR_CASE(2048) FR_CASE(4096) FR_CASE(8192)
 #undef FR_CASE
@@ -618,7 +631,7 @@ fresnel_status run_pass(fresnel_plan *p, void *wf, const PassSpec &q)
         a.inv_lambda = q.inv_lambda; a.scale = (float)q.scale; a.prefetch_distance = prefetch; a.pdl = p->pdl;
         a.lens2 = (const float2 *)q.lens2; a.mid2 = (const float2 *)q.mid2; a.amp2 = (const float *)q.amp2; a.opd2 = (const float *)q.opd2;
         switch (p->N) {
-#define FR_CASE(NN) case NN: e = tma ? launch_col_tma_f32_##NN(q.mode, a, p->tmap, *ma, *mo, p->batch, p->stream)           \
+#define FR_CASE(NN) case NN: e = tma ? launch_col_tma_f32_##NN(q.mode, a, wmap, *ma, *mo, p->batch, p->stream)           \
                                    : launch_pass_f32_##NN(q.col, q.mode, a, p->batch, p->stream); break;
             FR_CASE(64) FR_CASE(128) FR_CASE(256) FR_CASE(512) FR_CASE(1024) FR_CASE(2048) FR_CASE(4096) FR_CASE(8192)
 #undef FR_CASE
@@ -922,7 +935,8 @@ fresnel_status fresnel_plan_create(fresnel_plan **out, int N, int batch, fresnel
     p->map_descs.reserve(kMaxMapDescs);                            // pointers into it are handed out
     fresnel_status st;
     if (is_pow2(N)) {
-        p->tma_w = std::getenv("FRESNEL_NO_TMA") ? 0 : query_tma_width(N, dtype);     // env switch: A/B timing only
+        p->tma_w = std::getenv("FRESNEL_NO_TMA") ? 0 : query_tma_width(N, dtype, false);     // env switch: A/B timing only
+        p->tma_w2 = p->tma_w > 0 ? query_tma_width(N, dtype, true) : 0;
         p->map_box = query_map_box(N, dtype);
         st = upload_twiddles(p);
     } else {

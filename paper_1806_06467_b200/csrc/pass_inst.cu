@@ -57,10 +57,19 @@ cudaError_t FR_CAT(launch_col_tma_f64_, FR_N)(int mode, const PassArgs<double> &
     return tma_by_mode<double>(mode, a, m, ma, mo, batch, s);
 }
 // columns of a surface-map box of the fused column pass (the TMA minimum of 16 bytes may exceed the tile width)
-int FR_CAT(col_tma_map_box_f32_, FR_N)() { return MapTile<float, ColTmaGeom<float, FR_N>::W>::BOX_COLS; }
-int FR_CAT(col_tma_map_box_f64_, FR_N)() { return MapTile<double, ColTmaGeom<double, FR_N>::W>::BOX_COLS; }
-// columns per TMA tile (0: this N uses the per-thread-load column pass)
-int FR_CAT(col_tma_width_f32_, FR_N)() { return ColTmaGeom<float, FR_N>::supported ? ColTmaGeom<float, FR_N>::W : 0; }
-int FR_CAT(col_tma_width_f64_, FR_N)() { return ColTmaGeom<double, FR_N>::supported ? ColTmaGeom<double, FR_N>::W : 0; }
+int FR_CAT(col_tma_map_box_f32_, FR_N)() { return MapTile<float, ColTmaGeom<float, FR_N, true>::W>::BOX_COLS; }
+int FR_CAT(col_tma_map_box_f64_, FR_N)() { return MapTile<double, ColTmaGeom<double, FR_N, true>::W>::BOX_COLS; }
+// columns per TMA tile of the single-transform / single-convolution passes and of the fused pass (0: this N uses the
+// per-thread-load column pass)
+int FR_CAT(col_tma_width_f32_, FR_N)(bool conv2)
+{
+    if (!ColTmaGeom<float, FR_N>::supported) return 0;
+    return conv2 ? ColTmaGeom<float, FR_N, true>::W : ColTmaGeom<float, FR_N, false>::W;
+}
+int FR_CAT(col_tma_width_f64_, FR_N)(bool conv2)
+{
+    if (!ColTmaGeom<double, FR_N>::supported) return 0;
+    return conv2 ? ColTmaGeom<double, FR_N, true>::W : ColTmaGeom<double, FR_N, false>::W;
+}
 
 } // namespace fresnel

@@ -67,11 +67,14 @@ enum { FRESNEL_FORWARD = +1, FRESNEL_INVERSE = -1 };
  * device.  Builds the FFT twiddle tables (host long double, rounded once) and allocates the chirp
  * table cache.  batch >= 1.  *out is set only on FRESNEL_OK.  Grid sizes:
  *   - powers of two in [64, 8192]: the register-resident radix-16 kernels (the fast path; all BASELINE configs);
- *   - any other N in [16, 8192] ("N = 2800 ran faster than 4096"; npix = 1025, :259): the
- *     shared-memory path of gen_kernel.cuh -- mixed radix when N = 2^a 3^b 5^c 7^d 11^e 13^f, otherwise Bluestein
- *     (chirp x circular convolution of the next 7-smooth length >= 2N-1 x chirp), as long as two line buffers of the
- *     transform length fit one SM's shared memory (mixed radix N <= 6700, Bluestein N <= 3350 for both precisions;
- *     complex64 then takes 16-byte column tiles); beyond that FRESNEL_ERR_UNSUPPORTED.  Odd N: the grid
+ *   - N = 700, 1400, 2800 ("N = 2800 ran faster than 4096"): a register-resident mixed-radix pass
+ *     (mr_kernel.cuh; 2800 = 5 * 5 * 7 * 16), faster per step than N = 4096 here too;
+ *   - any other N in [16, 8192] (App. B calls WFIRSTSPC(npix=1025) at beam ratio 0.25, a 4100^2 grid):
+ *     the shared-memory path of gen_kernel.cuh -- mixed radix when N = 2^a 3^b 5^c 7^d 11^e 13^f [x one prime 17..61]
+ *     (1025 = 41 * 5^2, 4100 = 41 * 2^2 * 5^2), otherwise Bluestein (chirp x circular convolution of the next 7-smooth
+ *     length >= 2N-1 x chirp), as long as two line buffers of the transform length fit one SM's shared memory (mixed
+ *     radix N <= 6700, Bluestein N <= 3350 for both precisions; complex64 then takes 16-byte column tiles); beyond that
+ *     FRESNEL_ERR_UNSUPPORTED.  Odd N: the grid
  *     centre is pixel N/2 (integer division), frequencies in FFT order are q/(N dx) for q <= (N-1)/2 and
  *     (q-N)/(N dx) above, and centred transforms carry phase ramps instead of (-1)^n signs.  Train-level fusion
  *     (fresnel_system_run) applies to power-of-two grids only. */

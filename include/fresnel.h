@@ -67,8 +67,9 @@ enum { FRESNEL_FORWARD = +1, FRESNEL_INVERSE = -1 };
  * device.  Builds the FFT twiddle tables (host long double, rounded once) and allocates the chirp
  * table cache.  batch >= 1.  *out is set only on FRESNEL_OK.  Grid sizes:
  *   - powers of two in [64, 8192]: the register-resident radix-16 kernels (the fast path; all BASELINE configs);
- *   - N = 700, 1400, 2800 ("N = 2800 ran faster than 4096"): a register-resident mixed-radix pass
- *     (mr_kernel.cuh; 2800 = 5 * 5 * 7 * 16), faster per step than N = 4096 here too;
+ *   - N = 2800 ("N = 2800 ran faster than 4096") and 700, 1000, 1200, 1400, 1500, 2000, 2400, 3000, 3600,
+ *     4000, 5000, 5600, 6000: a register-resident mixed-radix pass (mr_kernel.cuh; 2800 = 5 * 5 * 7 * 16); N = 2800 is
+ *     faster per step than N = 4096 here too;
  *   - any other N in [16, 8192] (App. B calls WFIRSTSPC(npix=1025) at beam ratio 0.25, a 4100^2 grid):
  *     the shared-memory path of gen_kernel.cuh -- mixed radix when N = 2^a 3^b 5^c 7^d 11^e 13^f [x one prime 17..61]
  *     (1025 = 41 * 5^2, 4100 = 41 * 2^2 * 5^2), otherwise Bluestein (chirp x circular convolution of the next 7-smooth

@@ -20,6 +20,8 @@ OBJ = os.path.join(HERE, "build", os.environ.get("FRESNEL_LIB_NAME", "libfresnel
 LIB = os.path.join(HERE, os.environ.get("FRESNEL_LIB_NAME", "libfresnel.so"))
 EXTRA_DEFINES = os.environ.get("FRESNEL_DEFINES", "").split()
 SIZES = (64, 128, 256, 512, 1024, 2048, 4096, 8192)
+# grid sizes of the register-resident mixed-radix pass (mr_kernel.cuh; keep in step with FR_MR_SIZES of csrc/dispatch.h)
+MR_SIZES = (700, 1000, 1200, 1400, 1500, 2000, 2400, 2800, 3000, 3600, 4000, 5000, 5600, 6000)
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr"]
 
@@ -60,6 +62,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
         return LIB
     jobs = [(os.path.join(CSRC, "fresnel_api.cu"), os.path.join(OBJ, "fresnel_api.o"), [])]
     jobs.append((os.path.join(CSRC, "mr_inst.cu"), os.path.join(OBJ, "mr_inst.o"), []))
+    for n in MR_SIZES:
+        jobs.append((os.path.join(CSRC, "mr_inst.cu"), os.path.join(OBJ, f"mr_{n}.o"), [f"-DFR_MR_N={n}"]))
     for n in SIZES:
         jobs.append((os.path.join(CSRC, "pass_inst.cu"), os.path.join(OBJ, f"pass_{n}.o"), [f"-DFR_N={n}"]))
     with cf.ThreadPoolExecutor(max_workers=min(len(jobs), os.cpu_count() or 4)) as ex:

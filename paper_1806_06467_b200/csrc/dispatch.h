@@ -20,9 +20,15 @@ FR_DECL(64) FR_DECL(128) FR_DECL(256) FR_DECL(512) FR_DECL(1024) FR_DECL(2048) F
 #undef FR_DECL
 
 // register-resident mixed-radix pass (mr_kernel.cuh, instantiated in mr_inst.cu) for these grid sizes
-#define FR_MR_SIZES(X) X(700) X(1400) X(2800)
+#define FR_MR_SIZES(X) X(700) X(1000) X(1200) X(1400) X(1500) X(2000) X(2400) X(2800) X(3000) X(3600) X(4000) X(5000) X(5600) X(6000)
 template <typename T> struct GenArgs;
 cudaError_t launch_mr_f32(int N, bool col, int mode, const GenArgs<float> &a, const CUtensorMap &m, int batch, cudaStream_t s);
 cudaError_t launch_mr_f64(int N, bool col, int mode, const GenArgs<double> &a, const CUtensorMap &m, int batch, cudaStream_t s);
 int mr_col_width(int N, int elem_bytes);
+#define FR_DECL_MR(N)                                                                                                              \
+    cudaError_t launch_mr_f32_##N(bool col, int mode, const GenArgs<float> &a, const CUtensorMap &m, int batch, cudaStream_t s);   \
+    cudaError_t launch_mr_f64_##N(bool col, int mode, const GenArgs<double> &a, const CUtensorMap &m, int batch, cudaStream_t s);  \
+    int mr_col_width_##N(int elem_bytes);
+FR_MR_SIZES(FR_DECL_MR)
+#undef FR_DECL_MR
 } // namespace fresnel

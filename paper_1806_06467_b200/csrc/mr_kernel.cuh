@@ -22,20 +22,30 @@
 
 namespace fresnel {
 
-// forward stage order and threads per line of the supported sizes
+// Forward stage order and threads per line of the supported sizes: chosen (by exhaustive search over factorisations into
+// radices 2, 3, 4, 5, 7, 8, 16 and over TPL) for the fewest stages, then the fewest idle lanes, under "rounds x radix <= 16"
+// in every stage; odd radices first (a first stage of odd radix scatters without bank conflicts), the power of two last.
 template <int N> struct MrShape;
-template <> struct MrShape<2800> {
-    static constexpr int NST = 4, TPL = 200;
-    __host__ __device__ static constexpr int radix(int s) { constexpr int r[4] = {5, 5, 7, 16}; return r[s]; }
-};
-template <> struct MrShape<1400> {
-    static constexpr int NST = 4, TPL = 100;
-    __host__ __device__ static constexpr int radix(int s) { constexpr int r[4] = {5, 5, 7, 8}; return r[s]; }
-};
-template <> struct MrShape<700> {
-    static constexpr int NST = 4, TPL = 50;
-    __host__ __device__ static constexpr int radix(int s) { constexpr int r[4] = {5, 5, 7, 4}; return r[s]; }
-};
+#define FR_MR_SHAPE(NN, THREADS, STAGES, ...)                                                                        \
+    template <> struct MrShape<NN> {                                                                                 \
+        static constexpr int NST = STAGES, TPL = THREADS;                                                            \
+        __host__ __device__ static constexpr int radix(int s) { constexpr int r[STAGES] = {__VA_ARGS__}; return r[s]; } \
+    };
+FR_MR_SHAPE(700, 50, 4, 5, 5, 7, 4)
+FR_MR_SHAPE(1000, 125, 4, 5, 5, 5, 8)
+FR_MR_SHAPE(1200, 80, 4, 3, 5, 5, 16)
+FR_MR_SHAPE(1400, 100, 4, 5, 5, 7, 8)
+FR_MR_SHAPE(1500, 150, 5, 3, 5, 5, 5, 4)
+FR_MR_SHAPE(2000, 134, 4, 5, 5, 5, 16)
+FR_MR_SHAPE(2400, 160, 5, 3, 5, 5, 2, 16)
+FR_MR_SHAPE(2800, 200, 4, 5, 5, 7, 16)
+FR_MR_SHAPE(3000, 200, 5, 3, 5, 5, 5, 8)
+FR_MR_SHAPE(3600, 240, 5, 3, 3, 5, 5, 16)
+FR_MR_SHAPE(4000, 286, 5, 5, 5, 5, 2, 16)
+FR_MR_SHAPE(5000, 334, 5, 5, 5, 5, 5, 8)
+FR_MR_SHAPE(5600, 400, 5, 5, 5, 7, 2, 16)
+FR_MR_SHAPE(6000, 400, 5, 3, 5, 5, 5, 16)
+#undef FR_MR_SHAPE
 
 template <int N, int ORDER> __host__ __device__ constexpr int mr_radix(int s)
 {

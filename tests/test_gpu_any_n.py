@@ -4,8 +4,9 @@ memory, Bluestein for sizes with a large prime factor; mr_kernel.cuh: the regist
 N = 700, 1400, 2800) against the oracle's plain O(N^3) separable DFT, whole field, north-star tolerances + the max-abs
 bound.  Sizes: 100 = 2^2 5^2, 130 = 2 5 13, 175 = 5^2 7 (odd), 243 = 3^5 (odd), 335 = 5 67 (odd, Bluestein over
 M = 672), 360 = 2^3 3^2 5, 488 = 2^3 61 and 1025 = 5^2 41 (odd; one prime 17..61 as a direct first stage), 700 = 2^2 5^2 7
-(register-resident: partial butterfly rounds, a partial last TMA box), 1100 = 2^2 5^2 11, 1400 = 2^3 5^2 7,
-2800 = 2^4 5^2 7, 4100 = 2^2 5^2 41 (the paper's App. B call: npix = 1025 at beam ratio 0.25).
+(register-resident: partial butterfly rounds, a partial last TMA box), 1100 = 2^2 5^2 11, 1200 = 3 5 5 16 (register-resident with a
+radix-3 stage), 1400 = 2^3 5^2 7, 1500 and 2400 (register-resident in five stages), 2800 = 2^4 5^2 7, 4100 = 2^2 5^2 41 (the paper's
+App. B call: npix = 1025 at beam ratio 0.25); every register-resident size also against the shared-memory pass.
 """
 import math
 
@@ -16,7 +17,7 @@ from test_gpu_parity import TOL, assert_parity, field, map_dev, map_host, to_dev
 
 pytestmark = pytest.mark.gpu
 
-SIZES = [100, 130, 175, 243, 335, 360, 488, 700, 1025]
+SIZES = [100, 130, 175, 243, 335, 360, 488, 700, 1025, 1200]
 
 
 @pytest.fixture(scope="module")
@@ -137,11 +138,12 @@ def test_n2800_the_papers_size(torch_cuda, B, oracle, dtype):
 
 
 @pytest.mark.parametrize("dtype", ["c128", "c64"])
-def test_n1400_register_resident_all_modes(torch_cuda, B, oracle, dtype):
-    """N = 1400 = 5 * 5 * 7 * 8 on the register-resident mixed-radix pass (mr_kernel.cuh): inverse and centred transforms,
-    angular spectrum, direct Fresnel with z < 0, and a surface with both maps on the load of the row pass."""
+@pytest.mark.parametrize("N", [1400, 1500, 2400])
+def test_register_resident_all_modes(torch_cuda, B, oracle, N, dtype):
+    """N = 1400 = 5 * 5 * 7 * 8, 1500 = 3 * 5 * 5 * 5 * 4 and 2400 = 3 * 5 * 5 * 2 * 16 (five stages) on the register-resident
+    mixed-radix pass (mr_kernel.cuh): inverse and centred transforms, direct Fresnel with z < 0, and a surface with both maps
+    on the load of the row pass."""
     from paper_1806_06467_b200 import inputs
-    N = 1400
     u = field(N, 11500, 1, dtype)
     dx, lam = np.array([1.5e-5]), np.array([0.8e-6])
     zc = N * dx[0] ** 2 / lam[0]
@@ -195,6 +197,38 @@ def test_n4100_the_papers_appendix_b_grid(torch_cuda, B, oracle, dtype):
     d = to_dev(torch_cuda, w, dtype)
     plan.propagate_as(d, dxs, lams, zt / 2)
     assert_parity(d.cpu().numpy(), np.roll(w, (per // 2, per // 2), axis=(1, 2)), dtype, "half Talbot distance")
+
+
+MR_SIZES = [700, 1000, 1200, 1400, 1500, 2000, 2400, 2800, 3000, 3600, 4000, 5000, 5600, 6000]
+
+
+@pytest.mark.parametrize("dtype", ["c128", "c64"])
+@pytest.mark.parametrize("N", MR_SIZES)
+def test_register_resident_pass_equals_the_shared_memory_pass(torch_cuda, B, N, dtype):
+    """Cross-check (not the parity proof: that is the oracle at 700 ... 2800 above): at EVERY size of the register-resident
+    pass the results equal those of the shared-memory mixed-radix pass (FRESNEL_NO_MR=1 at plan creation), which the oracle
+    covers at many sizes -- angular spectrum, an inverse centred transform and direct Fresnel, to rounding."""
+    import os
+    u = field(N, 11700 + N, 1, dtype)
+    dx, lam = np.array([1.1e-5]), np.array([0.9e-6])
+    zc = N * dx[0] ** 2 / lam[0]
+    out = {}
+    for tag in ("fast", "shared"):
+        if tag == "shared":
+            os.environ["FRESNEL_NO_MR"] = "1"
+        try:
+            plan = B.Plan(N, 1, dtype)
+        finally:
+            os.environ.pop("FRESNEL_NO_MR", None)
+        res = []
+        d = to_dev(torch_cuda, u, dtype); plan.propagate_as(d, dx, lam, 0.3 * zc); res.append(d.cpu().numpy())
+        d = to_dev(torch_cuda, u, dtype); plan.fft2d(d, -1, True); res.append(d.cpu().numpy())
+        d = to_dev(torch_cuda, u, dtype); plan.propagate_direct(d, dx, lam, 1.3 * zc); res.append(d.cpu().numpy())
+        out[tag] = res
+        plan.close()
+    tol = 1e-13 if dtype == "c128" else 2e-6
+    for a, b, what in zip(out["fast"], out["shared"], ("angular spectrum", "inverse centred transform", "direct Fresnel")):
+        assert np.linalg.norm(a - b) / np.linalg.norm(b) <= tol, f"N = {N} {what}"
 
 
 def test_n1100_radix_11_and_capacity_limits(torch_cuda, B, oracle):

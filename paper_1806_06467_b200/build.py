@@ -61,6 +61,12 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if not force and os.path.exists(LIB) and os.path.exists(stamp) and open(stamp).read() == digest:
         return LIB
     jobs = [(os.path.join(CSRC, "fresnel_api.cu"), os.path.join(OBJ, "fresnel_api.o"), [])]
+    # the longest compilations first (the shared-memory pass: ~75 k instructions per instantiation)
+    for f64 in (1, 0):
+        for nt in (256, 512):
+            jobs.append((os.path.join(CSRC, "gen_inst.cu"), os.path.join(OBJ, f"gen_{'f64' if f64 else 'f32'}_{nt}.o"),
+                         [f"-DFR_GEN_F64={f64}", f"-DFR_GEN_NT={nt}"]))
+    jobs.append((os.path.join(CSRC, "gen_inst.cu"), os.path.join(OBJ, "gen_inst.o"), []))
     jobs.append((os.path.join(CSRC, "mr_inst.cu"), os.path.join(OBJ, "mr_inst.o"), []))
     for n in MR_SIZES:
         jobs.append((os.path.join(CSRC, "mr_inst.cu"), os.path.join(OBJ, f"mr_{n}.o"), [f"-DFR_MR_N={n}"]))

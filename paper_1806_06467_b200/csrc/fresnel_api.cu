@@ -587,7 +587,8 @@ template <typename T> cudaError_t run_generic(fresnel_plan *p, void *wf, const P
         if constexpr (sizeof(T) == 8) return launch_mr_f64(p->N, q.col, q.mode, a, p->tmap, p->batch, p->stream);
         else return launch_mr_f32(p->N, q.col, q.mode, a, p->tmap, p->batch, p->stream);
     }
-    return launch_gen_pass<T>(a, p->tmap, p->batch, gen_smem(p, a.W), p->stream);
+    if constexpr (sizeof(T) == 8) return launch_gen_pass_f64(a, p->tmap, p->batch, gen_smem(p, a.W), p->stream);
+    else return launch_gen_pass_f32(a, p->tmap, p->batch, gen_smem(p, a.W), p->stream);
 }
 
 fresnel_status run_pass(fresnel_plan *p, void *wf, const PassSpec &q)

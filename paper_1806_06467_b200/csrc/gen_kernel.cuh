@@ -440,21 +440,20 @@ __global__ void __launch_bounds__(NT, NT == kGenThreads ? 2 : 1) gen_pass_kernel
     }
 }
 
-template <typename T>
-cudaError_t launch_gen_pass(const GenArgs<T> &a, const CUtensorMap &tmap, int batch, size_t smem, cudaStream_t stream)
+// One (precision, CTA size) of the generic kernel: instantiated in gen_inst.cu, one object each (the kernel is ~75 k SASS
+// instructions per instantiation; four objects compile in parallel).
+template <typename T, int NT>
+cudaError_t launch_gen_pass_nt(const GenArgs<T> &a, const CUtensorMap &tmap, int batch, size_t smem, cudaStream_t stream)
 {
-    // two CTAs of kGenThreads per SM where their buffers fit, else one of twice the size
-    const bool two = 2 * (smem + 1024) <= (size_t)227 * 1024;
-    auto kern = two ? gen_pass_kernel<T, kGenThreads> : gen_pass_kernel<T, 2 * kGenThreads>;
+    auto kern = gen_pass_kernel<T, NT>;
     static std::atomic<unsigned long long> configured{0};
     if (fr_needs_configuring(configured)) {
-        cudaError_t e = cudaFuncSetAttribute(gen_pass_kernel<T, kGenThreads>, cudaFuncAttributeMaxDynamicSharedMemorySize, kGenMaxSmem);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(gen_pass_kernel<T, 2 * kGenThreads>, cudaFuncAttributeMaxDynamicSharedMemorySize, kGenMaxSmem);
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kGenMaxSmem);
         if (e != cudaSuccess) return e;
         fr_mark_configured(configured);
     }
     dim3 grid((a.N + a.W - 1) / a.W, batch, 1);
-    return launch_pdl(kern, grid, dim3(two ? kGenThreads : 2 * kGenThreads), smem, stream, a.pdl != 0, a, tmap);
+    return launch_pdl(kern, grid, dim3(NT), smem, stream, a.pdl != 0, a, tmap);
 }
 
 } // namespace fresnel

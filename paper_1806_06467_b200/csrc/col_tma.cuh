@@ -291,7 +291,7 @@ template <typename T, int N, bool CONV2 = false> struct ColTmaGeom {
     static constexpr int W = fr_tma_cols(N, ES, CONV2);
     static constexpr int threads = W * TL;
     static constexpr size_t smem = (size_t)W * fr_padded_len(N) * ES;
-    static constexpr int regs_goal = sizeof(T) == 8 ? FR_REGS_F64 : FR_REGS_F32;
+    static constexpr int regs_goal = sizeof(T) == 8 ? FR_REGS_F64 : (N <= 512 && FR_REGS_F32 < 72 ? 72 : FR_REGS_F32);   // as PassGeom
     static constexpr int minb_regs = 65536 / (threads * regs_goal);
     static constexpr int minb_smem = (int)((226 * 1024) / (smem + 1024));
     static constexpr int minb0 = minb_regs < minb_smem ? minb_regs : minb_smem;

@@ -249,9 +249,13 @@ col_tma_kernel(PassArgs<T> a, const __grid_constant__ CUtensorMap tmap, const __
     }
 
     __syncthreads();                                 // every group is done with its exchange buffer
+    // (the tile offsets are recomputed from an opaque copy of j: kept from the load they cost nine spilled registers that
+    // come back from local memory right here, at the end of the CTA's life)
+    int js = j;
+    asm volatile("" : "+r"(js));
 #pragma unroll
     for (int r = 0; r < 16; ++r) {
-        const uint32_t off = (uint32_t)((j + r * TL) * ROW_BYTES + g * ES);
+        const uint32_t off = (uint32_t)((js + r * TL) * ROW_BYTES + g * ES);
         *reinterpret_cast<C *>(tile + tile_swizzle<ROW_BYTES>(off)) = v[r];
     }
     fence_async_proxy();

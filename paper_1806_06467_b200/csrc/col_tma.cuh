@@ -105,7 +105,7 @@ FR_DEV void fetch_map_tile(unsigned char *tile, const CUtensorMap *mmap, uint64_
 // Fused column pass: where MINB resident CTAs still fit with it, the FIRST map of the in-between optic gets a
 // landing zone of its own behind the tile and is fetched at kernel start (it is an input, not a result of the
 // previous pass, so the fetch does not even wait for it): no bubble between the two convolutions.  Elsewhere
-// (N >= 4096) the map is fetched into the idle exchange space when it is needed.
+// (N >= 2048) the map is fetched into the idle exchange space when it is needed.
 template <typename T, int N, int W, int MINB> struct ColMapBuf {
     static constexpr int ES = (int)sizeof(typename cplx_of<T>::type);
     static constexpr size_t tile_bytes = ((size_t)W * fr_padded_len(N) * ES + 127) / 128 * 128;

@@ -47,7 +47,8 @@ def make_train(N, dx, seed):
 @pytest.mark.parametrize("N", [128, 512, 1024, 2048])
 def test_fused_train_matches_the_oracle(torch_cuda, B, oracle, N, dtype):
     """N = 128 takes the per-thread-load column pass, N >= 512 the TMA column pass (map tiles by TMA: early-fetched
-    into their own landing zone at N <= 2048); two wavelengths per call."""
+    into their own landing zone at N <= 1024, into the idle exchange space of the 16-byte-wide tiles at N = 2048); two
+    wavelengths per call."""
     dx = 2e-5
     surfs = make_train(N, dx, 9000 + N)
     u = field(N, 9100 + N, 2, dtype)

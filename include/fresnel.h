@@ -56,7 +56,8 @@ typedef enum {
     FRESNEL_ERR_INVALID_ARG = 1,
     FRESNEL_ERR_UNSUPPORTED = 2,
     FRESNEL_ERR_ALLOC = 3,
-    FRESNEL_ERR_CUDA = 4
+    FRESNEL_ERR_CUDA = 4,
+    FRESNEL_ERR_TOO_LARGE = 5      /* fresnel_mft_noalloc only: the problem exceeds its fixed scratch array */
 } fresnel_status;
 
 enum { FRESNEL_FORWARD = +1, FRESNEL_INVERSE = -1 };
@@ -254,6 +255,25 @@ fresnel_status fresnel_system_run_pilot(fresnel_plan *p, void *wf, double *pixel
 fresnel_status fresnel_plan_reserve_mft(fresnel_plan *p, int nb_max);
 fresnel_status fresnel_mft(fresnel_plan *p, const void *in, void *out, int nb, const double *pixel_in, const double *pixel_out,
                            const double *lambda, double f, int direction);
+
+/* The same transform for callers that may NOT allocate device memory (code under CUDA-graph capture, tight serving
+ * loops, harnesses that forbid cudaMalloc): no plan, no cudaMalloc / cudaFree / allocating library call on any path.
+ * The scratch of the two GEMMs (kernel matrix and intermediate) lives in one file-scope `static __device__` array of
+ * FIXED size inside the library -- 2 * FRESNEL_MFT_NOALLOC_MAX_ELEMS complex doubles = 8 MiB (+ 1.5 KiB of per-batch
+ * scalars) that every GPU that loads the library holds until the process exits.  Limits: batch * nb * na <=
+ * FRESNEL_MFT_NOALLOC_MAX_ELEMS (e.g. one 1024 -> 256 transform, four 512 -> 128 ones) and batch <=
+ * FRESNEL_MFT_NOALLOC_MAX_BATCH; anything larger is refused with FRESNEL_ERR_TOO_LARGE and nothing is enqueued.
+ * in: device, [batch][na][na] of `dtype`, read only; out: device, [batch][nb][nb] of `dtype`, written; must not alias.
+ * pixel_in / pixel_out / lambda: HOST arrays of `batch` doubles; f, direction: as fresnel_mft; stream: a cudaStream_t
+ * passed as void* (NULL = legacy default stream), on the CURRENT device.  Enqueues five kernels and returns (it does not
+ * synchronise); results equal fresnel_mft's bit for bit (same kernels).
+ * SHARED STATE: every call on a device uses the same array, which keeps the last call's contents.  Each call writes
+ * every word it later reads, so nothing needs clearing -- but two calls whose kernels can overlap on the GPU (different
+ * streams without an ordering between them, or two host threads) RACE on it: order them on one stream or by events. */
+#define FRESNEL_MFT_NOALLOC_MAX_ELEMS 262144
+#define FRESNEL_MFT_NOALLOC_MAX_BATCH 32
+fresnel_status fresnel_mft_noalloc(const void *in, void *out, int na, int nb, int batch, fresnel_dtype dtype, const double *pixel_in,
+                                   const double *pixel_out, const double *lambda, double f, int direction, void *stream);
 
 /* Broadband (polychromatic) image: the incoherent, weighted sum of the batch's monochromatic intensities
  * ("calculations must be repeated for all of the wavelengths"; one process per wavelength in

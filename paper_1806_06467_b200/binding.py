@@ -29,7 +29,7 @@ SYMBOLS = (
     "fresnel_plan_create", "fresnel_plan_set_stream", "fresnel_plan_synchronize", "fresnel_plan_destroy",
     "fresnel_plan_launch_count", "fresnel_plan_record_pass_events", "fresnel_plan_record_train_events",
     "fresnel_plan_last_schedule", "fresnel_plan_reserve_tables", "fresnel_plan_release_graph_tables", "fresnel_apply_qpf", "fresnel_apply_mask", "fresnel_fft2d",
-    "fresnel_propagate_as", "fresnel_propagate_direct", "fresnel_surface_as", "fresnel_system_run", "fresnel_system_run_pilot", "fresnel_plan_reserve_mft", "fresnel_mft", "fresnel_accumulate_intensity", "fresnel_memcpy_h2d",
+    "fresnel_propagate_as", "fresnel_propagate_direct", "fresnel_surface_as", "fresnel_system_run", "fresnel_system_run_pilot", "fresnel_plan_reserve_mft", "fresnel_mft", "fresnel_mft_noalloc", "fresnel_accumulate_intensity", "fresnel_memcpy_h2d",
     "fresnel_memcpy_d2h", "fresnel_status_string", "fresnel_version",
 )
 
@@ -92,6 +92,7 @@ def lib() -> ctypes.CDLL:
     L.fresnel_system_run_pilot.argtypes = [vp, vp, dp, dp, ctypes.POINTER(_Surface), ci, cd, ctypes.POINTER(_PilotState), ctypes.POINTER(ci)]
     L.fresnel_plan_reserve_mft.argtypes = [vp, ci]
     L.fresnel_mft.argtypes = [vp, vp, vp, ci, dp, dp, dp, cd, ci]
+    L.fresnel_mft_noalloc.argtypes = [vp, vp, ci, ci, ci, ci, dp, dp, dp, cd, ci, vp]
     L.fresnel_accumulate_intensity.argtypes = [vp, vp, dp, vp]
     L.fresnel_memcpy_h2d.argtypes = [vp, vp, vp, ctypes.c_size_t]
     L.fresnel_memcpy_d2h.argtypes = [vp, vp, vp, ctypes.c_size_t]
@@ -327,6 +328,32 @@ class Plan:
         nbytes = src.numel() * src.element_size()
         self._chk(lib().fresnel_memcpy_d2h(self._h, ctypes.c_void_p(dst_host.data_ptr()), ctypes.c_void_p(src.data_ptr()), nbytes),
                   "fresnel_memcpy_d2h")
+
+
+MFT_NOALLOC_MAX_ELEMS, MFT_NOALLOC_MAX_BATCH = 262144, 32      # FRESNEL_MFT_NOALLOC_MAX_* of include/fresnel.h
+
+
+def mft_noalloc(wf, out, pixel_in, pixel_out, lam, f: float, direction: int = FORWARD, stream=None) -> None:
+    """fresnel_mft_noalloc: the matrix Fourier transform without a plan and without any device allocation (its scratch is
+    a fixed array inside the library: batch * nb * na <= MFT_NOALLOC_MAX_ELEMS, batch <= MFT_NOALLOC_MAX_BATCH; calls that
+    overlap on the GPU race on it).  wf: CUDA tensor [batch][na][na] complex64 / complex128, out: [batch][nb][nb], same dtype."""
+    import torch
+    if wf.dtype not in (torch.complex64, torch.complex128) or out.dtype != wf.dtype:
+        raise ValueError("wf and out must be complex64 or complex128 tensors of the same dtype")
+    if not (wf.is_cuda and out.is_cuda and wf.is_contiguous() and out.is_contiguous()) or wf.dim() != 3 or out.dim() != 3:
+        raise ValueError("wf [batch][na][na] and out [batch][nb][nb] must be contiguous CUDA tensors")
+    batch, na, nb = int(wf.shape[0]), int(wf.shape[-1]), int(out.shape[-1])
+    if wf.shape[1] != na or tuple(out.shape) != (batch, nb, nb):
+        raise ValueError("wf must be [batch][na][na] and out [batch][nb][nb]")
+    _, pi = _darr(pixel_in, batch)
+    _, po = _darr(pixel_out, batch)
+    _, lp = _darr(lam, batch)
+    s = torch.cuda.current_stream(wf.device) if stream is None else stream
+    st = lib().fresnel_mft_noalloc(ctypes.c_void_p(wf.data_ptr()), ctypes.c_void_p(out.data_ptr()), na, nb, batch,
+                                   C128 if wf.dtype == torch.complex128 else C64, pi, po, lp, float(f), int(direction),
+                                   ctypes.c_void_p(s.cuda_stream))
+    if st != 0:
+        raise FresnelError(st, "fresnel_mft_noalloc")
 
 
 def run_surfaces(plan: Plan, wf, pixel, lam, surfaces: Sequence, maps=None) -> None:

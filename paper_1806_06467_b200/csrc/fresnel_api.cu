@@ -906,6 +906,7 @@ const char *fresnel_status_string(fresnel_status s)
     case FRESNEL_ERR_UNSUPPORTED: return "FRESNEL_ERR_UNSUPPORTED";
     case FRESNEL_ERR_ALLOC: return "FRESNEL_ERR_ALLOC";
     case FRESNEL_ERR_CUDA: return "FRESNEL_ERR_CUDA";
+    case FRESNEL_ERR_TOO_LARGE: return "FRESNEL_ERR_TOO_LARGE";
     }
     return "FRESNEL_ERR_UNKNOWN";
 }
@@ -1465,6 +1466,93 @@ fresnel_status fresnel_accumulate_intensity(fresnel_plan *p, const void *wf, con
         e = launch_intensity<double>((const double2 *)wf, (double *)image, weight, p->N, p->batch, p->sms, p->stream, &p->launches);
     else
         e = launch_intensity<float>((const float2 *)wf, (float *)image, weight, p->N, p->batch, p->sms, p->stream, &p->launches);
+    return e == cudaSuccess ? FRESNEL_OK : FRESNEL_ERR_CUDA;
+}
+
+} // extern "C"
+
+// ---- fresnel_mft_noalloc: the matrix Fourier transform for callers that may not allocate ------------------------------
+// fresnel_mft keeps its kernel matrix E and the intermediate T^t of its two GEMMs in plan-owned cudaMalloc memory.  Callers
+// that cannot call cudaMalloc (code under CUDA-graph capture, tight serving loops, harnesses that forbid it) get this variant:
+// no plan, and the same scratch in ONE file-scope device array of a fixed, modest size that every GPU that loads the
+// library holds until exit (8 MiB + 1.5 KiB).  In host code the array's NAME is a host-side stand-in, not a device address, so
+// its address is looked up once per device with cudaGetSymbolAddress (that device current) and only that pointer goes to
+// the kernels.  All calls share the array and it keeps the last call's contents: every word a call reads (kernel matrix,
+// intermediate, per-batch scalars) is written by the same call first, so nothing has to start at zero and nothing is
+// cleared; calls that overlap on the GPU (two streams, two host threads) race on it.
+namespace {
+
+constexpr size_t kMftStaticElems = FRESNEL_MFT_NOALLOC_MAX_ELEMS;      // complex doubles per region: batch * nb * na at most
+constexpr int kMftStaticBatch = FRESNEL_MFT_NOALLOC_MAX_BATCH;         // one mft_scalars_kernel launch carries 32
+static_assert(kMftStaticBatch <= 32, "the per-batch scalars travel in one kernel-parameter block of 32");
+// [0, E): kernel matrix   [E, 2E): intermediate T^t   then 6 * batch doubles: c_hi, c_lo, alpha.re, alpha.im, alpha (interleaved)
+static __device__ __align__(256) double2 fr_mft_static_scratch[2 * kMftStaticElems + 3 * kMftStaticBatch];
+
+// device address of the array on the current device: cudaGetSymbolAddress once per device ordinal (a second thread
+// racing here looks the same address up twice)
+cudaError_t mft_static_scratch(double2 **out)
+{
+    static std::atomic<double2 *> addr[64];
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= 64) return cudaErrorInvalidDevice;
+    double2 *p = addr[dev].load(std::memory_order_acquire);
+    if (p == nullptr) {
+        e = cudaGetSymbolAddress((void **)&p, fr_mft_static_scratch);
+        if (e != cudaSuccess) return e;
+        if (p == nullptr) return cudaErrorInvalidSymbol;
+        addr[dev].store(p, std::memory_order_release);
+    }
+    *out = p;
+    return cudaSuccess;
+}
+
+} // namespace
+
+extern "C" {
+
+fresnel_status fresnel_mft_noalloc(const void *in, void *out, int na, int nb, int batch, fresnel_dtype dtype, const double *pixel_in,
+                                   const double *pixel_out, const double *lambda, double f, int direction, void *stream)
+{
+    if (!in || !out || in == out || na <= 0 || nb <= 0 || batch <= 0) return FRESNEL_ERR_INVALID_ARG;
+    if (dtype != FRESNEL_C64 && dtype != FRESNEL_C128) return FRESNEL_ERR_UNSUPPORTED;
+    if (batch > kMftStaticBatch || (size_t)batch * (size_t)nb * (size_t)na > kMftStaticElems) return FRESNEL_ERR_TOO_LARGE;
+    if (!valid_positive(pixel_in, batch) || !valid_positive(pixel_out, batch) || !valid_positive(lambda, batch)) return FRESNEL_ERR_INVALID_ARG;
+    if (!std::isfinite(f) || f == 0.0 || (direction != FRESNEL_FORWARD && direction != FRESNEL_INVERSE)) return FRESNEL_ERR_INVALID_ARG;
+    double2 *scratch = nullptr;
+    if (mft_static_scratch(&scratch) != cudaSuccess) { cudaGetLastError(); return FRESNEL_ERR_CUDA; }
+    cudaStream_t s = (cudaStream_t)stream;
+    double2 *E = scratch, *T = scratch + kMftStaticElems;
+    double *scal = reinterpret_cast<double *>(scratch + 2 * kMftStaticElems);
+    double2 *alpha = reinterpret_cast<double2 *>(scal + 4 * (size_t)batch);
+    // per batch element, as in fresnel_mft: c = dx dx'/(lambda f) in turns (double-double), alpha = -+ i dx^2/(lambda f)
+    MftScalArgs sa;
+    sa.dst = scal; sa.batch = batch; sa.b0 = 0; sa.n = batch;
+    for (int b = 0; b < batch; ++b) {
+        const long double c = (long double)pixel_in[b] * (long double)pixel_out[b] / ((long double)lambda[b] * (long double)f);
+        const double hi = (double)c, lo = (double)(c - (long double)hi);
+        const double gq = (double)((long double)pixel_in[b] * (long double)pixel_in[b] / ((long double)lambda[b] * (long double)f));
+        sa.v[0][b] = hi; sa.v[1][b] = lo; sa.v[2][b] = 0.0; sa.v[3][b] = direction == FRESNEL_FORWARD ? -gq : gq;
+    }
+    mft_scalars_kernel<<<1, 32, 0, s>>>(sa);
+    mft_alpha_kernel<<<(batch + 127) / 128, 128, 0, s>>>(scal, alpha, batch);
+    MftMatrixArgs m;                                            // the kernel matrix is rebuilt by every call: the array is shared
+    m.out = E; m.na = na; m.nb = nb; m.batch = batch; m.sign = direction == FRESNEL_FORWARD ? -1 : +1;
+    m.c_hi = scal; m.c_lo = scal + batch;
+    mft_matrix_kernel<<<dim3((na + 255) / 256, nb, batch), 256, 0, s>>>(m);
+    if (cudaGetLastError() != cudaSuccess) return FRESNEL_ERR_CUDA;
+    MftGemmArgs g1;                                             // T^t[q,j] = sum_k U[j,k] E[q,k]
+    g1.A = in; g1.B = E; g1.C = T; g1.M = na; g1.N = nb; g1.K = na;
+    g1.strideA = (size_t)na * na; g1.strideB = (size_t)nb * na; g1.strideC = (size_t)nb * na; g1.alpha = nullptr;
+    cudaError_t e = dtype == FRESNEL_C128 ? launch_mft_gemm<double2, double2, true>(g1, batch, s)
+                                          : launch_mft_gemm<float2, double2, true>(g1, batch, s);
+    if (e != cudaSuccess) return FRESNEL_ERR_CUDA;
+    MftGemmArgs g2;                                             // V[p,q] = alpha sum_j E[p,j] T^t[q,j]
+    g2.A = E; g2.B = T; g2.C = out; g2.M = nb; g2.N = nb; g2.K = na;
+    g2.strideA = (size_t)nb * na; g2.strideB = (size_t)nb * na; g2.strideC = (size_t)nb * nb; g2.alpha = alpha;
+    e = dtype == FRESNEL_C128 ? launch_mft_gemm<double2, double2, false>(g2, batch, s)
+                              : launch_mft_gemm<double2, float2, false>(g2, batch, s);
     return e == cudaSuccess ? FRESNEL_OK : FRESNEL_ERR_CUDA;
 }
 

@@ -35,7 +35,9 @@
  *                                         or a call needs more chirp-table slots than are free (all taken by
  *                                         captured graphs: see fresnel_plan_reserve_tables)
  *                FRESNEL_ERR_CUDA         a CUDA runtime call or launch failed
- *   Threads:   a plan is not thread-safe; distinct plans are independent.
+ *                FRESNEL_ERR_TOO_LARGE    fresnel_mft_noalloc only: the problem exceeds its fixed scratch array
+ *   Threads:   a plan is not thread-safe; distinct plans are independent.  fresnel_mft_noalloc has no plan and shares
+ *              one scratch array per device among all its calls (see there).
  *   There is no CPU fallback: without a CUDA device plan creation fails with FRESNEL_ERR_CUDA.
  */
 #ifndef FRESNEL_H
